@@ -1,0 +1,181 @@
+/*
+ * nhplan.h -- C ABI of libnhplan.so: the kernel-style N-turn planner of
+ * "Nonholonomic Motion Planning as Efficient as Piano Mover's" (arXiv 2306.01301) on one B200.
+ *
+ * Citations are lines of /root/reference/PAPER.md ("PAPER.md:<line>", with section / equation);
+ * "DESIGN R<k>" is a numbered reading in /root/repo/DESIGN.md section 3.
+ *
+ * The pipeline behind these calls is the paper's 8-step algorithm (section XI):
+ *   obstacle image -> [nhp_render_obstacles: steps 3-4] -> [nhp_run_nturn: step 5]
+ *   -> [nhp_extract_path: steps 6-8] -> plan on the host.
+ * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.  The library
+ * never allocates after nhp_planner_create ("no memory allocation takes place during processing",
+ * PAPER.md:565) and enqueues all work on the caller's stream; only nhp_extract_path, nhp_status and
+ * nhp_debug_tables synchronise that stream.
+ *
+ * Grid: N x N spatial cells (N = 2^log2_n) and N_theta = 2^log2_ntheta headings,
+ * Theta <-> angle 2 pi Theta / N_theta, all indices taken modulo their dimension, one-cell hard wall
+ * at i = 0 and j = 0.  Volume index idx = (Theta * N + j) * N + i  (i = x fastest).
+ * Vertex (i, j, Theta) stands for the pose (i + Psi0(Theta), j + Psi1(Theta), theta(Theta)), eq (16) l.256.
+ *
+ * Maneuver ids, in the paper's cycle order:
+ *   0 LF left-forward, 1 SF straight-forward, 2 RB right-backward,
+ *   3 RF right-forward, 4 SB straight-backward, 5 LB left-backward.
+ *
+ * Costs (DESIGN R18): uint32 fixed point, unit = 2^-cost_one_log2 cell of travel.  A finite cost is
+ * < NHP_COST_LIMIT = 2^30; a sum that reaches the limit saturates to NHP_INF.  Blocked and unreached
+ * vertices read NHP_INF in the exported volume.
+ *
+ * Thread safety: one handle <-> one stream <-> one caller thread at a time.
+ */
+#ifndef NHPLAN_H
+#define NHPLAN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NHP_INF 0xFFFFFFFFu
+#define NHP_COST_LIMIT (1u << 30)
+
+/* flags of nhp_weights.flags */
+#define NHP_FLAG_FORWARD_ONLY 1   /* Dubins car: only LF, SF, RF are swept */
+#define NHP_FLAG_SOFT 2           /* a soft-cost volume S is rendered and used */
+#define NHP_FLAG_SIMPLE_KERNELS 4 /* thread-per-curve bring-up kernels (the paper's own mapping, l.356);
+                                     same results, kept for A/B measurements */
+
+/* error codes (all entry points return 0 on success) */
+#define NHP_OK 0
+#define NHP_E_ARG (-1)            /* NULL / out-of-range argument */
+#define NHP_E_NOT_POW2 (-2)       /* log2 sizes outside [5, 12] x [5, 12] */
+#define NHP_E_ANGRES (-3)         /* N_theta < 2 pi R (DESIGN R23) */
+#define NHP_E_START_BLOCKED (-4)  /* the start vertex collides */
+#define NHP_E_GOAL_UNREACHED (-5) /* back-tracking found no finite predecessor */
+#define NHP_E_BUFFER (-6)         /* caller buffer too small / missing */
+#define NHP_E_CUDA (-7)           /* a CUDA call failed; see nhp_last_error */
+#define NHP_E_STATE (-8)          /* call out of order (e.g. run before render) */
+#define NHP_E_WEIGHTS (-9)        /* a cost weight is too large for the 2^30 cost range */
+
+typedef struct nhp_planner nhp_planner;
+
+/* Cost weights (DESIGN R8, R9).
+ *   ct[m]       transition cost charged on ENTERING maneuver m from the transition state, cost units, < 2^26
+ *   dir_mult[m] Q8.8 multiplier on the edge length of maneuver m (256 = 1.0; 512 on LB,SB,RB = "reverse x2")
+ * Edge leaving vertex p under maneuver m costs (len_q[m][Theta_p] * S[p]) >> 4 with
+ * len_q = round(2^cost_one_log2 * length * dir_mult / 256), length = 2 pi R / N_theta for turns and
+ * 1/|cos| or 1/|sin| for straights, S[p] = 16 without NHP_FLAG_SOFT. */
+typedef struct nhp_weights {
+    uint32_t ct[6];
+    uint32_t dir_mult[6];
+    int32_t cost_one_log2;   /* 0..16, 10 is the default used by the benchmarks */
+    int32_t flags;
+} nhp_weights;
+
+typedef struct nhp_sizes {
+    size_t V_bytes;          /* value volume, uint32 per vertex            (one volume) */
+    size_t C_bytes;          /* collision volume, 1 bit per vertex             */
+    size_t S_bytes;          /* soft volume, uint8 per vertex; 0 without NHP_FLAG_SOFT  */
+    size_t workspace_bytes;  /* scratch; may be 0                                                       */
+} nhp_sizes;
+
+/* Caller-owned DEVICE buffers (e.g. torch tensors), 256-byte aligned, alive until nhp_planner_destroy. */
+typedef struct nhp_buffers {
+    void *V;                 /* V_bytes */
+    void *C;                 /* C_bytes: word (Theta*N + j)*N/32 + i/32, bit i%32 = vertex (i,j,Theta) collides */
+    void *S;                 /* S_bytes or NULL: Q4.4 speed-reciprocal of vertex idx, >= 16 */
+    void *workspace;         /* workspace_bytes or NULL */
+} nhp_buffers;
+
+/* One transition point of a plan ("plan"): the vertex and the maneuver that ARRIVES at it
+ * from the next record; the last record is the start and has m = -1. */
+typedef struct nhp_waypoint {
+    int32_t i, j, theta, m;
+} nhp_waypoint;
+
+/* Sizes of the caller-owned buffers for a grid.  Pure host arithmetic. */
+int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, nhp_sizes *out);
+
+/* ini(R, cT, Lx, Lt) of PAPER.md:1169.  Builds the integer tables of section V.C (beta, Psi, B, I, J,
+ * edge lengths) on the host in fp64 once and uploads them.
+ *   R_cells      minimum turn radius in cells, >= 1; N_theta >= 2 pi R is enforced
+ *   dev          caller-owned device buffers (see nhp_buffers); S may be NULL without NHP_FLAG_SOFT
+ *   cuda_stream  a cudaStream_t (0 = legacy default stream) on the current device
+ * Errors: NHP_E_ARG, NHP_E_NOT_POW2, NHP_E_ANGRES, NHP_E_WEIGHTS, NHP_E_BUFFER, NHP_E_CUDA. */
+int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_cells,
+                       const nhp_weights *w, const nhp_buffers *dev, void *cuda_stream);
+
+int nhp_planner_destroy(nhp_planner *p);
+
+/* Static string describing the last error on this handle (never NULL). */
+const char *nhp_last_error(const nhp_planner *p);
+
+/* Vehicle shape (Figure 6 l.110: "the vehicle bounding shape can be arbitrary").
+ *   mask_host  HOST array, mh rows x mw columns, non-zero = vehicle; column p runs along the vehicle's
+ *              length axis u, row q along its width axis v
+ *   origin_u/v mask pixel (p, q) owns the vehicle-frame unit square centred (p - origin_u, q - origin_v);
+ *              the vehicle frame's origin is the centre of the rear axle
+ * Rasterises, per Theta, the set E_Theta of image-pixel offsets covered by the footprint of a pose
+ * (DESIGN R15: a pixel is covered iff its centre, rotated into the vehicle frame with Q14 integer
+ * cos/sin, falls in a set mask pixel; the half-cell pose offset Psi of eq (16) is applied, l.259).
+ * The footprint's circumscribed radius must be < N/2 - 2.  Errors: NHP_E_ARG, NHP_E_CUDA. */
+int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int mw, int mh,
+                                 double origin_u, double origin_v);
+
+/* Obstacle rendering, steps 3-4 of PAPER.md:390-391 (section VI l.338, appendix C l.871).
+ *   hard  N x N uint8 image, row = y (j), column = x (i); non-zero = hard obstacle
+ *   soft  N x N uint8 Q4.4 speed-reciprocal image (16 = 1.0) or NULL; requires NHP_FLAG_SOFT
+ *   on_device  0: both pointers are HOST memory and are copied to the device on the stream (step 3);
+ *              1: both are DEVICE pointers
+ * Writes C (bit = footprint at that pose touches a hard pixel, or a pixel of the wall a = 0 / b = 0 with
+ * toroidal image addressing, or i = 0, or j = 0) and, with soft, S = clamp(max of soft over the
+ * footprint, 16, 255) (DESIGN R16).  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_CUDA. */
+int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *soft, int on_device);
+
+/* Step 5 of PAPER.md:392: V <- INF, V[start] <- 0, then n_cycles maneuver cycles LF, SF, RB, RF, SB, LB
+ * (PAPER.md:475), each an in-place min-plus sweep of every curve of that maneuver (Inserts
+ * 3-5 l.922-949) gated by C and weighted by S.  n_cycles <= 0 selects the paper's default of 8.
+ * A blocked start is reported by the next nhp_extract_path / nhp_status (the check runs on the device).
+ * Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_CUDA. */
+int nhp_run_nturn(nhp_planner *p, int i, int j, int theta, int n_cycles);
+
+/* Continue sweeping the existing value volume for n_cycles more cycles. */
+int nhp_run_more(nhp_planner *p, int n_cycles);
+
+/* Cost-to-come volume in canonical form: uint32 [Theta][j][i], NHP_INF on blocked / unreached vertices.
+ * *dev_ptr_out is the caller's own V buffer (borrowed, DEVICE), valid until the next run / destroy.  The
+ * conversion from the sweeps' internal encoding is enqueued on the stream (one pass over V). */
+int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out);
+
+/* Steps 6-8 of PAPER.md:393-395 with an explicit goal vertex (DESIGN R20): repeated reverse Bellman step
+ * over the six whole curves through the current vertex, eq (32) l.380; ties resolve to the earliest
+ * maneuver in cycle order, then to the nearest source (DESIGN R19).
+ *   out_host  HOST array of cap records, filled goal -> start
+ *   count     number of records written;  cost: sum over segments of ct[m] + edge weights
+ * Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_START_BLOCKED, NHP_E_GOAL_UNREACHED,
+ * NHP_E_BUFFER (plan longer than cap), NHP_E_CUDA. */
+int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *out_host, int cap,
+                     int *count, uint32_t *cost);
+
+/* Synchronise and report device-side conditions of the last run (NHP_OK or NHP_E_START_BLOCKED). */
+int nhp_status(nhp_planner *p);
+
+/* eq (16) PAPER.md:256 and its inverse (nearest vertex). x, y in cells, theta in radians. */
+int nhp_index_to_pose(const nhp_planner *p, int i, int j, int theta, double *x, double *y, double *theta_rad);
+int nhp_pose_to_index(const nhp_planner *p, double x, double y, double theta_rad, int *i, int *j, int *theta);
+
+/* Debug accessor: copies the library's tables to HOST arrays (any pointer may be NULL).
+ *   beta int32[N_theta], psi2 uint8[N_theta] (= 2 Psi), B int32[N_theta][N], I uint8[N_theta],
+ *   J int8[N_theta], len_q uint32[6][N_theta] */
+int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t *B, uint8_t *I, int8_t *J,
+                     uint32_t *len_q);
+
+/* Number of kernels launched by this handle since creation (for bench.py's gpu_launches). */
+long long nhp_launch_count(const nhp_planner *p);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NHPLAN_H */

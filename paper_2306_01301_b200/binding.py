@@ -1,0 +1,220 @@
+"""ctypes binding with the same names as the C ABI (include/nhplan.h)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnhplan.so")
+
+INF = 0xFFFFFFFF
+FLAG_FORWARD_ONLY, FLAG_SOFT, FLAG_SIMPLE_KERNELS = 1, 2, 4
+MANEUVER_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB")
+ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_START_BLOCKED",
+          -5: "NHP_E_GOAL_UNREACHED", -6: "NHP_E_BUFFER", -7: "NHP_E_CUDA", -8: "NHP_E_STATE", -9: "NHP_E_WEIGHTS"}
+
+EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
+           "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_run_nturn", "nhp_run_more",
+           "nhp_cost_volume", "nhp_extract_path", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
+           "nhp_debug_tables", "nhp_launch_count")
+
+
+class Weights(C.Structure):
+    _fields_ = [("ct", C.c_uint32 * 6), ("dir_mult", C.c_uint32 * 6), ("cost_one_log2", C.c_int32), ("flags", C.c_int32)]
+
+
+class Sizes(C.Structure):
+    _fields_ = [("V_bytes", C.c_size_t), ("C_bytes", C.c_size_t), ("S_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
+
+
+class Buffers(C.Structure):
+    _fields_ = [("V", C.c_void_p), ("C", C.c_void_p), ("S", C.c_void_p), ("workspace", C.c_void_p)]
+
+
+class Waypoint(C.Structure):
+    _fields_ = [("i", C.c_int32), ("j", C.c_int32), ("theta", C.c_int32), ("m", C.c_int32)]
+
+
+class NhpError(RuntimeError):
+    def __init__(self, code, msg=""):
+        super().__init__(f"{ERRORS.get(code, code)}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libnhplan.so; fails loudly if it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2306_01301_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(_LIB_PATH)
+        L.nhp_query_sizes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Sizes)]
+        L.nhp_planner_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_double, C.POINTER(Weights),
+                                         C.POINTER(Buffers), C.c_void_p]
+        L.nhp_planner_destroy.argtypes = [C.c_void_p]
+        L.nhp_last_error.argtypes = [C.c_void_p]
+        L.nhp_last_error.restype = C.c_char_p
+        L.nhp_render_vehicle_footprint.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.nhp_render_obstacles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.nhp_run_more.argtypes = [C.c_void_p, C.c_int]
+        L.nhp_cost_volume.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.nhp_extract_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Waypoint), C.c_int,
+                                       C.POINTER(C.c_int), C.POINTER(C.c_uint32)]
+        L.nhp_status.argtypes = [C.c_void_p]
+        L.nhp_index_to_pose.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int] + [C.POINTER(C.c_double)] * 3
+        L.nhp_pose_to_index.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double] + [C.POINTER(C.c_int)] * 3
+        L.nhp_debug_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        L.nhp_launch_count.argtypes = [C.c_void_p]
+        L.nhp_launch_count.restype = C.c_longlong
+        _lib = L
+    return _lib
+
+
+def query_sizes(log2_n, log2_ntheta, flags=0):
+    s = Sizes()
+    rc = load_library().nhp_query_sizes(log2_n, log2_ntheta, flags, C.byref(s))
+    if rc:
+        raise NhpError(rc, "query_sizes")
+    return s
+
+
+class Planner:
+    """One planner handle = one grid, one stream.  Method names follow the C ABI without the nhp_ prefix."""
+
+    def __init__(self, log2_n, log2_ntheta, R, ct, dir_mult=(256,) * 6, cost_one_log2=10, flags=0, device="cuda:0",
+                 stream=None):
+        import torch
+        self._L = load_library()
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2306_01301_b200.Planner needs a CUDA device; there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.n, self.nt = 1 << log2_n, 1 << log2_ntheta
+        self.shape = (self.nt, self.n, self.n)
+        self.flags = flags
+        sz = query_sizes(log2_n, log2_ntheta, flags)
+        with torch.cuda.device(self.device):
+            self.V = torch.empty(sz.V_bytes // 4, dtype=torch.int32, device=self.device)
+            self.C = torch.empty(sz.C_bytes // 4, dtype=torch.int32, device=self.device)
+            self.S = torch.empty(sz.S_bytes, dtype=torch.uint8, device=self.device) if sz.S_bytes else None
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            w = Weights((C.c_uint32 * 6)(*ct), (C.c_uint32 * 6)(*dir_mult), cost_one_log2, flags)
+            b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None, None)
+            h = C.c_void_p()
+            rc = self._L.nhp_planner_create(C.byref(h), log2_n, log2_ntheta, float(R), C.byref(w), C.byref(b),
+                                            C.c_void_p(self.stream.cuda_stream))
+        if rc:
+            raise NhpError(rc, "planner_create")
+        self._h = h
+
+    @classmethod
+    def from_scene(cls, sc, flags=0, **kw):
+        f = flags | sc.flags | (FLAG_SOFT if sc.soft is not None else 0)
+        p = cls(sc.log2_n, sc.log2_nt, sc.R, sc.ct, sc.dir_mult, sc.cost_one_log2, f, **kw)
+        p.render_vehicle_footprint(sc.mask, sc.ou, sc.ov)
+        return p
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.nhp_planner_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc, what):
+        if rc:
+            raise NhpError(rc, f"{what}: {self._L.nhp_last_error(self._h).decode()}")
+
+    # ---- the ABI calls ---------------------------------------------------------------------
+    def render_vehicle_footprint(self, mask, origin_u, origin_v):
+        mask = np.ascontiguousarray(mask, np.uint8)
+        self._check(self._L.nhp_render_vehicle_footprint(self._h, mask.ctypes.data, mask.shape[1], mask.shape[0],
+                                                         float(origin_u), float(origin_v)), "render_vehicle_footprint")
+
+    def render_obstacles(self, hard, soft=None):
+        """hard / soft: numpy uint8 arrays or CPU torch tensors (host path, copied inside the call) or CUDA tensors."""
+        def ptr(a):
+            if a is None:
+                return None, 0
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.uint8 and a.flags.c_contiguous and a.shape == (self.n, self.n)
+                return a.ctypes.data, 0
+            assert a.dtype == self.torch.uint8 and a.is_contiguous() and tuple(a.shape) == (self.n, self.n)
+            return a.data_ptr(), int(a.is_cuda)
+        hp, hd = ptr(hard)
+        sp, sd = ptr(soft)
+        assert soft is None or hd == sd
+        self._keep = (hard, soft)                       # host buffers must outlive the async copy
+        self._check(self._L.nhp_render_obstacles(self._h, hp, sp, hd), "render_obstacles")
+
+    def run_nturn(self, start, n_cycles=8):
+        self._check(self._L.nhp_run_nturn(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_cycles)), "run_nturn")
+
+    def run_more(self, n_cycles):
+        self._check(self._L.nhp_run_more(self._h, int(n_cycles)), "run_more")
+
+    def cost_volume(self):
+        """Canonical cost-to-come volume as a (N_theta, N, N) int32 CUDA tensor view of V (bit pattern = uint32)."""
+        out = C.c_void_p()
+        self._check(self._L.nhp_cost_volume(self._h, C.byref(out)), "cost_volume")
+        assert out.value == self.V.data_ptr()
+        return self.V.view(self.shape)
+
+    def extract_path(self, goal, cap=4096):
+        buf = (Waypoint * cap)()
+        cnt, cost = C.c_int(0), C.c_uint32(0)
+        self._check(self._L.nhp_extract_path(self._h, int(goal[0]), int(goal[1]), int(goal[2]), buf, cap,
+                                             C.byref(cnt), C.byref(cost)), "extract_path")
+        return [(w.i, w.j, w.theta, w.m) for w in buf[:cnt.value]], cost.value
+
+    def status(self):
+        self._check(self._L.nhp_status(self._h), "status")
+
+    def index_to_pose(self, i, j, theta):
+        x, y, t = C.c_double(), C.c_double(), C.c_double()
+        self._check(self._L.nhp_index_to_pose(self._h, i, j, theta, C.byref(x), C.byref(y), C.byref(t)), "index_to_pose")
+        return x.value, y.value, t.value
+
+    def pose_to_index(self, x, y, theta_rad):
+        i, j, t = C.c_int(), C.c_int(), C.c_int()
+        self._check(self._L.nhp_pose_to_index(self._h, x, y, theta_rad, C.byref(i), C.byref(j), C.byref(t)), "pose_to_index")
+        return i.value, j.value, t.value
+
+    def debug_tables(self):
+        n, nt = self.n, self.nt
+        t = dict(beta=np.empty(nt, np.int32), psi2=np.empty(nt, np.uint8), B=np.empty((nt, n), np.int32),
+                 I=np.empty(nt, np.uint8), J=np.empty(nt, np.int8), len_q=np.empty((6, nt), np.uint32))
+        self._check(self._L.nhp_debug_tables(self._h, *[t[k].ctypes.data for k in ("beta", "psi2", "B", "I", "J", "len_q")]),
+                    "debug_tables")
+        return t
+
+    def launch_count(self):
+        return int(self._L.nhp_launch_count(self._h))
+
+    # ---- host copies for tests ---------------------------------------------------------------
+    def cost_volume_numpy(self):
+        return self.cost_volume().cpu().numpy().view(np.uint32)
+
+    def collision_numpy(self):
+        """Unpacked collision volume, uint8 {0,1} [Theta][j][i]."""
+        words = self.C.cpu().numpy().view(np.uint32)
+        bits = np.unpackbits(words.view(np.uint8), bitorder="little")
+        return bits.reshape(self.shape)
+
+    def soft_numpy(self):
+        return None if self.S is None else self.S.cpu().numpy().reshape(self.shape)

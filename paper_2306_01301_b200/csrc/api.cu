@@ -1,0 +1,325 @@
+// C ABI of libnhplan.so (include/nhplan.h): argument checking, host-side table build
+// and kernel launches.  No planning arithmetic runs on the host after nhp_planner_create.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "nhp_internal.cuh"
+
+namespace {
+
+constexpr double kPi = 3.14159265358979323846;
+
+int fail(nhp_planner *p, int code, const char *what)
+{
+    if (p) p->err = what;
+    return code;
+}
+
+int cuda_fail(nhp_planner *p, cudaError_t e, const char *where)
+{
+    if (p) p->err = std::string(where) + ": " + cudaGetErrorString(e);
+    return NHP_E_CUDA;
+}
+
+#define CU(call)                                                   \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(p, e_, #call);     \
+    } while (0)
+
+// sin(2 pi k / nt), argument reduced to the first octant in integers so that the symmetries the paper
+// relies on (Psi_2 = Psi_0, Psi_3 = Psi_1; tan = +-1 exactly on the diagonals, DESIGN R5)
+// hold bit for bit.
+double sin_frac(int k, int nt)
+{
+    const int half = nt / 2, q = nt / 4;
+    k &= nt - 1;
+    double sign = 1.0;
+    if (k >= half) { k -= half; sign = -1.0; }
+    if (k > q) k = half - k;
+    double s;
+    if (k == 0) s = 0.0;
+    else if (k == q) s = 1.0;
+    else if (2 * k <= q) s = std::sin(2.0 * kPi * (double)k / (double)nt);
+    else s = std::cos(2.0 * kPi * (double)(q - k) / (double)nt);
+    return sign * s;
+}
+
+// Section V.C of the paper, evaluated once in fp64 and frozen into integer tables.
+int build_tables(nhp_planner *p)
+{
+    const int n = p->n, nt = p->nt;
+    p->beta.resize(nt); p->psi2.resize(nt); p->I.resize(nt); p->J.resize(nt);
+    p->B.resize((size_t)nt * n); p->len_q.resize((size_t)6 * nt); p->cosq.resize(nt); p->sinq.resize(nt);
+    const double one = (double)(1u << p->w.cost_one_log2);
+    for (int t = 0; t < nt; t++) {
+        const double s = sin_frac(t, nt), c = sin_frac(t + nt / 4, nt);
+        // alpha = R sin(theta); zeta(x) = round(2x)/2; beta = floor(zeta(alpha)); Psi = zeta - beta  (l.233-240)
+        const double z = std::round(2.0 * (p->R * s)) / 2.0;
+        const double fl = std::floor(z);
+        p->beta[t] = (int32_t)fl;
+        p->psi2[t] = (uint8_t)(int)(2.0 * (z - fl));
+        // eq (19) on the integer octant; eq (20); eq (24)
+        const int o = t & (nt / 2 - 1);
+        const int I = (o <= nt / 8 || o >= 3 * nt / 8) ? 0 : 1;
+        const double K = I == 0 ? s / c : c / s, f = I == 0 ? c : s;
+        p->I[t] = (uint8_t)I;
+        p->J[t] = (int8_t)(f > 0 ? 1 : -1);
+        for (int y = 0; y < n; y++) p->B[(size_t)t * n + y] = (int32_t)std::round((double)y * K);   // l.284
+        // edge lengths l.334 -> fixed point
+        const double lt = 2.0 * kPi * p->R / (double)nt, ls = 1.0 / std::fabs(f);
+        for (int m = 0; m < 6; m++) {
+            const double len = (m == M_SF || m == M_SB) ? ls : lt;
+            const double q = std::round(one * len * (double)p->w.dir_mult[m] / 256.0);
+            if (q < 1.0 || q * 255.0 / 16.0 >= (double)(1u << 26)) return NHP_E_WEIGHTS;
+            p->len_q[(size_t)m * nt + t] = (uint32_t)q;
+        }
+        p->cosq[t] = (int32_t)std::round(16384.0 * c);
+        p->sinq[t] = (int32_t)std::round(16384.0 * s);
+    }
+    for (int m = 0; m < 6; m++)
+        if (p->w.ct[m] >= (1u << 26)) return NHP_E_WEIGHTS;
+    return NHP_OK;
+}
+
+int upload_tables(nhp_planner *p)
+{
+    const int n = p->n, nt = p->nt;
+    std::vector<int16_t> beta16(nt), B16((size_t)nt * n);
+    std::vector<uint8_t> IJ(nt);
+    std::vector<int32_t> rot((size_t)4 * nt);
+    for (int t = 0; t < nt; t++) {
+        beta16[t] = (int16_t)p->beta[t];
+        IJ[t] = (uint8_t)(p->I[t] | ((p->J[t] > 0 ? 1 : 0) << 1));
+        rot[4 * t + 0] = p->cosq[t]; rot[4 * t + 1] = p->sinq[t];
+        rot[4 * t + 2] = p->psi2[t]; rot[4 * t + 3] = p->psi2[(t + nt / 4) & (nt - 1)];   // 2 Psi0, 2 Psi1, eq (16)
+    }
+    for (size_t k = 0; k < B16.size(); k++) B16[k] = (int16_t)p->B[k];
+    CU(cudaMalloc(&p->d_beta, sizeof(int16_t) * nt));
+    CU(cudaMalloc(&p->d_B, sizeof(int16_t) * B16.size()));
+    CU(cudaMalloc(&p->d_lenq, sizeof(uint32_t) * 6 * nt));
+    CU(cudaMalloc(&p->d_IJ, nt));
+    CU(cudaMalloc(&p->d_rot, sizeof(int32_t) * 4 * nt));
+    CU(cudaMemcpyAsync(p->d_beta, beta16.data(), sizeof(int16_t) * nt, cudaMemcpyHostToDevice, p->stream));
+    CU(cudaMemcpyAsync(p->d_B, B16.data(), sizeof(int16_t) * B16.size(), cudaMemcpyHostToDevice, p->stream));
+    CU(cudaMemcpyAsync(p->d_lenq, p->len_q.data(), sizeof(uint32_t) * 6 * nt, cudaMemcpyHostToDevice, p->stream));
+    CU(cudaMemcpyAsync(p->d_IJ, IJ.data(), nt, cudaMemcpyHostToDevice, p->stream));
+    CU(cudaMemcpyAsync(p->d_rot, rot.data(), sizeof(int32_t) * 4 * nt, cudaMemcpyHostToDevice, p->stream));
+    CU(cudaStreamSynchronize(p->stream));            // the staging vectors die with this scope
+    return NHP_OK;
+}
+
+bool in_grid(const nhp_planner *p, int i, int j, int t) { return i >= 0 && j >= 0 && t >= 0 && i < p->n && j < p->n && t < p->nt; }
+
+}  // namespace
+
+extern "C" {
+
+int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, nhp_sizes *out)
+{
+    if (!out) return NHP_E_ARG;
+    if (log2_n < 5 || log2_n > 12 || log2_ntheta < 5 || log2_ntheta > 12) return NHP_E_NOT_POW2;
+    const size_t nr = ((size_t)1 << (2 * log2_n)) << log2_ntheta;
+    out->V_bytes = nr * 4;
+    out->C_bytes = nr / 8;
+    out->S_bytes = (flags & NHP_FLAG_SOFT) ? nr : 0;
+    out->workspace_bytes = 0;
+    return NHP_OK;
+}
+
+int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_cells, const nhp_weights *w,
+                       const nhp_buffers *dev, void *cuda_stream)
+{
+    if (!out || !w || !dev) return NHP_E_ARG;
+    *out = nullptr;
+    if (log2_n < 5 || log2_n > 12 || log2_ntheta < 5 || log2_ntheta > 12) return NHP_E_NOT_POW2;
+    if (!(R_cells >= 1.0) || w->cost_one_log2 < 0 || w->cost_one_log2 > 16) return NHP_E_ARG;
+    if ((double)(1 << log2_ntheta) < 2.0 * kPi * R_cells) return NHP_E_ANGRES;
+    if (!dev->V || !dev->C || ((w->flags & NHP_FLAG_SOFT) && !dev->S)) return NHP_E_BUFFER;
+    if (((uintptr_t)dev->V | (uintptr_t)dev->C | (uintptr_t)dev->S) & 255) return NHP_E_BUFFER;
+    nhp_planner *p = new (std::nothrow) nhp_planner();
+    if (!p) return NHP_E_ARG;
+    p->log2_n = log2_n; p->log2_nt = log2_ntheta; p->n = 1 << log2_n; p->nt = 1 << log2_ntheta;
+    p->R = R_cells; p->w = *w; p->stream = (cudaStream_t)cuda_stream;
+    p->V = (uint32_t *)dev->V; p->C = (uint32_t *)dev->C; p->S = (w->flags & NHP_FLAG_SOFT) ? (uint8_t *)dev->S : nullptr;
+    int rc = build_tables(p);
+    if (rc == NHP_OK) rc = upload_tables(p);
+    const size_t npx = (size_t)p->n * p->n;
+    p->plan_cap = 4096;
+    auto alloc = [&](void **ptr, size_t bytes) { if (rc == NHP_OK && cudaMalloc(ptr, bytes) != cudaSuccess) rc = NHP_E_CUDA; };
+    alloc((void **)&p->d_hard, npx);
+    alloc((void **)&p->d_soft, npx);
+    alloc((void **)&p->d_H, npx / 8);
+    alloc((void **)&p->d_status, sizeof(int32_t) * 8);
+    alloc((void **)&p->d_plan, sizeof(nhp_waypoint) * p->plan_cap);
+    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * 8) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_plan, sizeof(nhp_waypoint) * p->plan_cap) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK && cudaMemsetAsync(p->d_status, 0, sizeof(int32_t) * 8, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc != NHP_OK) { nhp_planner_destroy(p); return rc; }
+    *out = p;
+    return NHP_OK;
+}
+
+int nhp_planner_destroy(nhp_planner *p)
+{
+    if (!p) return NHP_E_ARG;
+    cudaStreamSynchronize(p->stream);
+    cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot);
+    cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_H);
+    cudaFree(p->d_status); cudaFree(p->d_plan);
+    if (p->h_status) cudaFreeHost(p->h_status);
+    if (p->h_plan) cudaFreeHost(p->h_plan);
+    delete p;
+    return NHP_OK;
+}
+
+const char *nhp_last_error(const nhp_planner *p) { return p ? p->err.c_str() : "null handle"; }
+
+int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int mw, int mh, double origin_u, double origin_v)
+{
+    if (!p || !mask_host || mw < 1 || mh < 1 || mw > 1024 || mh > 1024) return fail(p, NHP_E_ARG, "bad footprint mask");
+    // circumscribed radius of the mask around the vehicle origin, in cells (+2 for Psi and rounding)
+    const double mu = std::fmax(std::fabs(-origin_u - 0.5), std::fabs((double)mw - 1.0 - origin_u + 0.5));
+    const double mv = std::fmax(std::fabs(-origin_v - 0.5), std::fabs((double)mh - 1.0 - origin_v + 0.5));
+    const int rad = (int)std::ceil(std::hypot(mu, mv)) + 2;
+    if (2 * rad >= p->n) return fail(p, NHP_E_ARG, "footprint does not fit the grid");
+    p->have_footprint = false;
+    CU(cudaStreamSynchronize(p->stream));
+    cudaFree(p->d_mask); cudaFree(p->d_E);
+    p->d_mask = nullptr; p->d_E = nullptr;
+    p->rad = rad; p->side = 2 * rad + 1; p->sidew = (p->side + 31) / 32;
+    CU(cudaMalloc(&p->d_mask, (size_t)mw * mh));
+    CU(cudaMalloc(&p->d_E, sizeof(uint32_t) * (size_t)p->nt * p->side * p->sidew));
+    CU(cudaMemcpyAsync(p->d_mask, mask_host, (size_t)mw * mh, cudaMemcpyHostToDevice, p->stream));
+    const int64_t ouq = (int64_t)std::llround(origin_u * 32768.0), ovq = (int64_t)std::llround(origin_v * 32768.0);
+    p->launches += launch_footprint_raster(p, mw, mh, ouq, ovq);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(p->stream));            // mask_host may be freed by the caller after return
+    p->have_footprint = true;
+    p->have_render = false;
+    return NHP_OK;
+}
+
+int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *soft, int on_device)
+{
+    if (!p || !hard) return fail(p, NHP_E_ARG, "hard image is NULL");
+    if (!p->have_footprint) return fail(p, NHP_E_STATE, "render_obstacles before render_vehicle_footprint");
+    const bool want_soft = p->S != nullptr;
+    if (want_soft && !soft) return fail(p, NHP_E_ARG, "NHP_FLAG_SOFT planner needs a soft image");
+    if (!want_soft && soft) return fail(p, NHP_E_ARG, "soft image given but the planner has no soft volume");
+    const size_t npx = (size_t)p->n * p->n;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(p->d_hard, hard, npx, kind, p->stream));                       // step 3
+    if (want_soft) CU(cudaMemcpyAsync(p->d_soft, soft, npx, kind, p->stream));
+    p->launches += launch_render(p, want_soft);                                       // step 4
+    CU(cudaGetLastError());
+    p->have_render = true;
+    p->have_run = false;
+    return NHP_OK;
+}
+
+int nhp_run_nturn(nhp_planner *p, int i, int j, int theta, int n_cycles)
+{
+    if (!p) return NHP_E_ARG;
+    if (!p->have_render) return fail(p, NHP_E_STATE, "run_nturn before render_obstacles");
+    if (!in_grid(p, i, j, theta)) return fail(p, NHP_E_ARG, "start pose outside the grid");
+    if (n_cycles <= 0) n_cycles = 8;
+    p->start[0] = i; p->start[1] = j; p->start[2] = theta;
+    p->launches += launch_init_volume(p, i, j, theta);
+    p->canonical = false;
+    p->launches += launch_cycles(p, n_cycles);
+    CU(cudaGetLastError());
+    p->have_run = true;
+    return NHP_OK;
+}
+
+int nhp_run_more(nhp_planner *p, int n_cycles)
+{
+    if (!p) return NHP_E_ARG;
+    if (!p->have_run) return fail(p, NHP_E_STATE, "run_more before run_nturn");
+    if (n_cycles <= 0) return fail(p, NHP_E_ARG, "n_cycles must be positive");
+    if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
+    p->launches += launch_cycles(p, n_cycles);
+    CU(cudaGetLastError());
+    return NHP_OK;
+}
+
+int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out)
+{
+    if (!p || !dev_ptr_out) return NHP_E_ARG;
+    if (!p->have_run) return fail(p, NHP_E_STATE, "cost_volume before run_nturn");
+    if (!p->canonical) { p->launches += launch_export_volume(p, true); p->canonical = true; }
+    CU(cudaGetLastError());
+    *dev_ptr_out = p->V;
+    return NHP_OK;
+}
+
+int nhp_status(nhp_planner *p)
+{
+    if (!p) return NHP_E_ARG;
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    if (p->have_run && p->h_status[0]) return fail(p, NHP_E_START_BLOCKED, "the start vertex collides");
+    return NHP_OK;
+}
+
+int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *out_host, int cap, int *count, uint32_t *cost)
+{
+    if (!p || !out_host || !count || !cost || cap < 1) return fail(p, NHP_E_ARG, "bad extract_path argument");
+    if (!p->have_run) return fail(p, NHP_E_STATE, "extract_path before run_nturn");
+    if (!in_grid(p, gi, gj, gtheta)) return fail(p, NHP_E_ARG, "goal pose outside the grid");
+    *count = 0; *cost = NHP_INF;
+    if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
+    p->launches += launch_backtrack(p, gi, gj, gtheta);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));                                             // step 8
+    const int rc = p->h_status[1];
+    if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
+    if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "goal not reached");
+    if (rc != NHP_OK) return fail(p, rc, "plan longer than the internal buffer");
+    const int n = p->h_status[2];
+    if (n > cap) return fail(p, NHP_E_BUFFER, "plan longer than the caller's buffer");
+    std::memcpy(out_host, p->h_plan, sizeof(nhp_waypoint) * n);
+    *count = n;
+    *cost = (uint32_t)p->h_status[3];
+    return NHP_OK;
+}
+
+int nhp_index_to_pose(const nhp_planner *p, int i, int j, int theta, double *x, double *y, double *theta_rad)
+{
+    if (!p || !x || !y || !theta_rad || !in_grid(p, i, j, theta)) return NHP_E_ARG;
+    *x = i + p->psi2[theta] / 2.0;                                                    // eq (16)
+    *y = j + p->psi2[(theta + p->nt / 4) & (p->nt - 1)] / 2.0;
+    *theta_rad = 2.0 * kPi * theta / p->nt;
+    return NHP_OK;
+}
+
+int nhp_pose_to_index(const nhp_planner *p, double x, double y, double theta_rad, int *i, int *j, int *theta)
+{
+    if (!p || !i || !j || !theta) return NHP_E_ARG;
+    const int t = (int)std::llround(theta_rad / (2.0 * kPi) * p->nt) & (p->nt - 1);
+    const long long ii = std::llround(x - p->psi2[t] / 2.0), jj = std::llround(y - p->psi2[(t + p->nt / 4) & (p->nt - 1)] / 2.0);
+    if (ii < 0 || jj < 0 || ii >= p->n || jj >= p->n) return NHP_E_ARG;
+    *i = (int)ii; *j = (int)jj; *theta = t;
+    return NHP_OK;
+}
+
+int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t *B, uint8_t *I, int8_t *J, uint32_t *len_q)
+{
+    if (!p) return NHP_E_ARG;
+    if (beta) std::memcpy(beta, p->beta.data(), sizeof(int32_t) * p->nt);
+    if (psi2) std::memcpy(psi2, p->psi2.data(), p->nt);
+    if (B) std::memcpy(B, p->B.data(), sizeof(int32_t) * p->B.size());
+    if (I) std::memcpy(I, p->I.data(), p->nt);
+    if (J) std::memcpy(J, p->J.data(), p->nt);
+    if (len_q) std::memcpy(len_q, p->len_q.data(), sizeof(uint32_t) * p->len_q.size());
+    return NHP_OK;
+}
+
+long long nhp_launch_count(const nhp_planner *p) { return p ? p->launches : 0; }
+
+}  // extern "C"

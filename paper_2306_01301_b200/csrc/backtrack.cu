@@ -1,0 +1,168 @@
+// Back-tracking.  PAPER.md:376-382 (section X): "Each step of back-tracking is
+// doing a Bellman-iteration in reverse ... back-tracing through all the maneuver curves that go through
+// the current vertex in their entirety ... adding edge values sequentially and comparing the running sum
+// plus the value of each vertex to the minimum so far", eq (32) l.380.  It is "like running the maneuver
+// kernel in reverse, but for only one curve for each maneuver" -- so one block does it: warp m walks the
+// curve of maneuver m through the current vertex, 32 vertices per step (addresses come straight from
+// the curve maps (18)/(23), so nothing in the walk is a dependent load), with a warp prefix sum for E_sum
+// and a warp arg-min.  Tie rule DESIGN R19: earliest maneuver in cycle order, then nearest source.
+#include "nhp_internal.cuh"
+
+struct BtParams {
+    uint32_t ct[6];
+    int log2_n, nt, fwd_only, soft;
+    int si, sj, st, gi, gj, gt;
+    int cap;
+};
+
+__device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long x)
+{
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        const unsigned long long y = __shfl_xor_sync(0xffffffffu, x, d);
+        x = y < x ? y : x;
+    }
+    return x;
+}
+
+__global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restrict__ V, const uint8_t *__restrict__ S,
+                                                       DevTables T, BtParams P, nhp_waypoint *__restrict__ plan,
+                                                       int32_t *__restrict__ status)
+{
+    __shared__ unsigned long long s_key[6];     // (candidate cost << 13) | steps back
+    __shared__ uint32_t s_seg[6];               // ct + E_sum of the winning candidate
+    __shared__ int s_cell[6][3];
+    __shared__ int s_cur[4];                    // i, j, theta, continue flag
+    const int m = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int log2_n = P.log2_n, n = 1 << log2_n, mx = n - 1, nt = P.nt, mt = nt - 1, quarter = nt >> 2;
+    const unsigned long long KINF = ~0ull;
+    int cnt = 0;
+    unsigned long long total = 0;
+    if (threadIdx.x == 0) {
+        int go = 1;
+        const size_t gidx = ((((size_t)P.gt << log2_n) + P.gj) << log2_n) + P.gi;
+        if (status[0]) { status[1] = NHP_E_START_BLOCKED; go = 0; }
+        else if (V[gidx] == 0u) { status[1] = NHP_E_GOAL_UNREACHED; go = 0; }
+        else if (P.gi == P.si && P.gj == P.sj && P.gt == P.st) {
+            if (P.cap < 1) status[1] = NHP_E_BUFFER;
+            else { plan[0] = nhp_waypoint{P.gi, P.gj, P.gt, -1}; status[1] = NHP_OK; status[2] = 1; status[3] = 0; }
+            go = 0;
+        }
+        s_cur[0] = P.gi; s_cur[1] = P.gj; s_cur[2] = P.gt; s_cur[3] = go;
+    }
+    __syncthreads();
+    while (s_cur[3]) {
+        const int ci = s_cur[0], cj = s_cur[1], cth = s_cur[2];
+        const bool turn = !(m == M_SF || m == M_SB);
+        const bool skip = P.fwd_only && (m == M_RB || m == M_SB || m == M_LB);
+        unsigned long long best = KINF;
+        uint32_t best_seg = 0;
+        int bi = 0, bj = 0, bt = 0;
+        if (!skip) {
+            // thread coordinates of the curve through the current vertex: inverse of (18) / (23), eq (29)
+            int xp, yp, qa = 0, qb = 0, up;
+            const int16_t *Bt = T.B + (size_t)cth * n;
+            const int I = T.IJ[cth] & 1, jpos = (T.IJ[cth] >> 1) & 1;
+            if (turn) {
+                const bool left = (m == M_LF || m == M_LB);
+                qa = left ? 0 : 2; qb = left ? 3 : 1;
+                xp = (ci - T.beta[(cth + qa * quarter) & mt]) & mx;
+                yp = (cj - T.beta[(cth + qb * quarter) & mt]) & mx;
+                up = (m == M_LF || m == M_RB);
+            } else {
+                yp = I ? cj : ci;
+                xp = ((I ? ci : cj) - Bt[yp]) & mx;
+                up = ((m == M_SF) == (jpos == 1));
+            }
+            const int maxk = turn ? nt - 1 : n;
+            const uint32_t ct = P.ct[m];
+            unsigned long long E = 0;
+            for (int base = 0; base < maxk; base += 32) {
+                const int k = base + lane + 1;                 // steps back, against the direction of m
+                int i, j, t;
+                if (turn) {
+                    t = (up ? cth - k : cth + k) & mt;
+                    i = (xp + T.beta[(t + qa * quarter) & mt]) & mx;
+                    j = (yp + T.beta[(t + qb * quarter) & mt]) & mx;
+                } else {
+                    const int y = (up ? yp - k : yp + k) & mx;
+                    const int c = (xp + Bt[y]) & mx;
+                    t = cth; i = I ? c : y; j = I ? y : c;
+                }
+                const size_t idx = ((((size_t)t << log2_n) + j) << log2_n) + i;
+                const bool valid = k <= maxk;
+                const uint32_t u = valid ? V[idx] : 0u;
+                const unsigned blk = __ballot_sync(0xffffffffu, u == 0u);       // blocked (or past the end)
+                const int first = blk ? __ffs(blk) - 1 : 32;
+                uint32_t w = T.len_q[(size_t)m * nt + t];
+                if (P.soft) w = (w * (uint32_t)(valid ? S[idx] : 16)) >> 4;
+                unsigned long long pre = (lane < first) ? w : 0;                 // inclusive prefix sum of w
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const unsigned long long y = __shfl_up_sync(0xffffffffu, pre, d);
+                    if (lane >= d) pre += y;
+                }
+                pre += E;
+                unsigned long long key = KINF;
+                uint32_t seg = 0;
+                if (lane < first && u < VI_INF) {
+                    const unsigned long long cand = (unsigned long long)(u - 1u) + ct + pre;
+                    if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ct + pre); }
+                }
+                const unsigned long long kmin = warp_min_u64(key);
+                if (kmin < best) {                               // strictly smaller: earlier chunks win ties
+                    best = kmin;
+                    const unsigned who = __ballot_sync(0xffffffffu, key == kmin);
+                    const int src = __ffs(who) - 1;
+                    best_seg = __shfl_sync(0xffffffffu, seg, src);
+                    bi = __shfl_sync(0xffffffffu, i, src);
+                    bj = __shfl_sync(0xffffffffu, j, src);
+                    bt = __shfl_sync(0xffffffffu, t, src);
+                }
+                E = __shfl_sync(0xffffffffu, pre, 31);
+                if (first < 32) break;
+            }
+        }
+        if (lane == 0) { s_key[m] = best; s_seg[m] = best_seg; s_cell[m][0] = bi; s_cell[m][1] = bj; s_cell[m][2] = bt; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int bm = -1;
+            unsigned long long bc = KINF;
+            for (int q = 0; q < 6; q++) {
+                const unsigned long long c = s_key[q] == KINF ? KINF : (s_key[q] >> 13);
+                if (c < bc) { bc = c; bm = q; }
+            }
+            if (bm < 0) { status[1] = NHP_E_GOAL_UNREACHED; s_cur[3] = 0; }
+            else if (cnt >= P.cap) { status[1] = NHP_E_BUFFER; s_cur[3] = 0; }
+            else {
+                plan[cnt++] = nhp_waypoint{ci, cj, cth, bm};
+                total += s_seg[bm];
+                s_cur[0] = s_cell[bm][0]; s_cur[1] = s_cell[bm][1]; s_cur[2] = s_cell[bm][2];
+                if (s_cur[0] == P.si && s_cur[1] == P.sj && s_cur[2] == P.st) {
+                    if (cnt >= P.cap) status[1] = NHP_E_BUFFER;
+                    else {
+                        plan[cnt++] = nhp_waypoint{P.si, P.sj, P.st, -1};
+                        status[1] = NHP_OK; status[2] = cnt;
+                        status[3] = (int32_t)(total >= NHP_COST_LIMIT ? NHP_INF : (uint32_t)total);
+                    }
+                    s_cur[3] = 0;
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+int launch_backtrack(nhp_planner *p, int gi, int gj, int gt)
+{
+    BtParams P;
+    for (int m = 0; m < 6; m++) P.ct[m] = p->w.ct[m];
+    P.log2_n = p->log2_n; P.nt = p->nt;
+    P.fwd_only = (p->w.flags & NHP_FLAG_FORWARD_ONLY) ? 1 : 0;
+    P.soft = (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) ? 1 : 0;
+    P.si = p->start[0]; P.sj = p->start[1]; P.st = p->start[2];
+    P.gi = gi; P.gj = gj; P.gt = gt;
+    P.cap = p->plan_cap;
+    backtrack_kernel<<<1, 192, 0, p->stream>>>(p->V, p->S, p->tables(), P, p->d_plan, p->d_status);
+    return 1;
+}

@@ -1,0 +1,75 @@
+// Internal declarations of libnhplan.so (CUDA path).  Shares nothing with oracle/.
+// Citations: PAPER.md = /root/reference/PAPER.md; DESIGN R<k> = readings in /root/repo/DESIGN.md.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/nhplan.h"
+
+// ---- internal value encoding of the volume V while sweeps run -------------
+//   0            vertex is blocked (stamped from the collision bits by the init kernel)
+//   1 .. 2^30    cost + 1 of a reached vertex
+//   VI_INF       free vertex not reached yet
+// Any in-register value >= VI_INF means "infinite"; min(arrival, stored) therefore never needs a
+// clamp: blocked cells keep 0, unreached cells keep VI_INF, and nothing above VI_INF is ever stored.
+constexpr uint32_t VI_INF = (1u << 30) + 1u;
+constexpr uint32_t VI_BIG = VI_INF;            // added on edges that leave a blocked vertex
+
+enum { M_LF = 0, M_SF = 1, M_RB = 2, M_RF = 3, M_SB = 4, M_LB = 5 };
+
+struct DevTables {
+    const int16_t *beta;    // [nt]      beta(Theta), eq (13)-(17) PAPER.md:233-262
+    const int16_t *B;       // [nt][n]   B(y',Theta) = round(y' K(Theta))
+    const uint32_t *len_q;  // [6][nt]   fixed-point edge length
+    const uint8_t *IJ;      // [nt]      bit0 = I(Theta) eq (19), bit1 = (J(Theta) > 0) eq (24)
+};
+
+struct nhp_planner {
+    int log2_n = 0, log2_nt = 0, n = 0, nt = 0;
+    double R = 0;
+    nhp_weights w{};
+    cudaStream_t stream = nullptr;
+    uint32_t *V = nullptr, *C = nullptr;
+    uint8_t *S = nullptr;
+    // host tables (fp64 once, then integers)
+    std::vector<int32_t> beta, B, cosq, sinq;
+    std::vector<uint8_t> psi2, I;
+    std::vector<int8_t> J;
+    std::vector<uint32_t> len_q;
+    // device tables (library-owned, small)
+    int16_t *d_beta = nullptr, *d_B = nullptr;
+    uint32_t *d_lenq = nullptr;
+    uint8_t *d_IJ = nullptr;
+    int32_t *d_rot = nullptr;      // [nt][4] cosq, sinq, 2*Psi0, 2*Psi1
+    // footprint
+    int rad = 0, side = 0, sidew = 0;
+    uint8_t *d_mask = nullptr;
+    uint32_t *d_E = nullptr;       // [nt][side][sidew] bitmap of covered pixel offsets, bit (da + rad)
+    bool have_footprint = false;
+    // images
+    uint8_t *d_hard = nullptr, *d_soft = nullptr;
+    uint32_t *d_H = nullptr;       // [n][n/32] hard | wall, bit-packed rows
+    bool have_render = false, have_run = false, canonical = false;
+    int start[3] = {0, 0, 0};
+    // plan extraction
+    int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost
+    nhp_waypoint *d_plan = nullptr;
+    int plan_cap = 0;
+    int32_t *h_status = nullptr;   // pinned
+    nhp_waypoint *h_plan = nullptr;
+    std::string err = "ok";
+    long long launches = 0;
+
+    DevTables tables() const { return DevTables{d_beta, d_B, d_lenq, d_IJ}; }
+};
+
+// ---- kernel launchers (each returns the number of kernels it launched) ---------------------------
+int launch_footprint_raster(nhp_planner *p, int mw, int mh, int64_t ouq, int64_t ovq);
+int launch_render(nhp_planner *p, bool soft);
+int launch_init_volume(nhp_planner *p, int si, int sj, int st);
+int launch_export_volume(nhp_planner *p, bool to_canonical);
+int launch_cycles(nhp_planner *p, int n_cycles);
+int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);
