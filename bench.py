@@ -1,0 +1,304 @@
+"""bench.py -- one JSON line for the N-turn planner hot path on B200 (contract: see DESIGN.md section 9).
+
+A "step" is one pass of the whole hot path over one synthetic scene:
+    render_obstacles (collision [+ soft] volume)  ->  run_nturn (N_T maneuver cycles)  ->  extract_path
+`value`  = pose-updates / s with the obstacle images already resident in HBM (6 * N_T * N_R pose-updates per plan,
+           PAPER.md:453), whole job over all ranks (replicas only: one independent plan per GPU, no collective);
+`e2e`    = the same metric through the public API with HOST (pinned) obstacle images: the H2D copy of the images
+           and the D2H copy of the plan are inside the timed region;
+`roofline` = the dominant kernel's algorithmic bytes / its average CUDA-event duration over the timed region,
+           against the measured HBM copy bandwidth in MEASURED_PEAKS.json;
+`cpu_baseline` = the CPU oracle, as it stands, on a bounded sample of the same workload on this box's host cores.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl ours|reference]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "pose_updates_per_sec (N-turn planner, whole plan: render + N_T maneuver cycles + back-track)"
+UNIT = "Gpose-updates/s"
+FALLBACK_HBM_GBS = 6650.0            # /opt/skills/guides/B200_PROFILING.md fallback
+ALG_BYTES_HARD, ALG_BYTES_SOFT = 8.125, 9.125     # read V 4 + write V 4 + 1 collision bit [+ 1 soft byte]
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[k-1]; 3 = 512^3 maze (default)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cycles", type=int, default=0, help="override N_T (0 = the config's own)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--simple-kernels", action="store_true", help="thread-per-curve bring-up kernels (A/B)")
+    return ap.parse_args()
+
+
+def workload_name(sc, n_cycles):
+    return (f"{sc.name}: {sc.n}x{sc.n}x{sc.nt} (x,y,theta), vehicle {sc.mask.shape[1]}x{sc.mask.shape[0]}, R={sc.R:g}, "
+            f"N_T={n_cycles}, {'soft+hard' if sc.soft is not None else 'hard'} obstacles")
+
+
+def peak_hbm():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def pick_goal(p, sc, torch):
+    """The nominal goal if the sweeps reached it, else the reached candidate of largest finite cost
+    (N_T cycles only guarantee plans of <= N_T maneuvers).  Harness logic on <= 257 values."""
+    cands = [sc.goal] + list(sc.extra_goals)
+    V = p.cost_volume()
+    idx = torch.tensor([(t * sc.n + j) * sc.n + i for (i, j, t) in cands], device=V.device)
+    vals = V.view(-1)[idx].to(torch.int64) & 0xFFFFFFFF
+    vals = vals.cpu().tolist()
+    if vals[0] != 0xFFFFFFFF:
+        return tuple(sc.goal)
+    best = max(range(len(cands)), key=lambda k: (-1 if vals[k] == 0xFFFFFFFF else vals[k]))
+    return tuple(cands[best]) if vals[best] != 0xFFFFFFFF else tuple(sc.start)
+
+
+def run_ours(args):
+    import torch
+
+    import paper_2306_01301_b200 as nhp
+    import scenes
+    from paper_2306_01301_b200 import replicas
+
+    rank, local_rank, ws = replicas.init("nccl")
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    sc = scenes.CONFIGS[args.config](replicas.replica_seed(args.config, rank))
+    n_cycles = args.cycles or sc.n_cycles
+    n_r = sc.n * sc.n * sc.nt
+    updates_per_plan = 6 * n_cycles * n_r
+    p = nhp.Planner.from_scene(sc, flags=nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0, device=dev)
+    hard_d = torch.from_numpy(sc.hard).to(dev)
+    soft_d = torch.from_numpy(sc.soft).to(dev) if sc.soft is not None else None
+    hard_h = torch.from_numpy(sc.hard).pin_memory()
+    soft_h = torch.from_numpy(sc.soft).pin_memory() if sc.soft is not None else None
+    state = {"goal": tuple(sc.goal), "plan": None}
+
+    def step(hard, soft):
+        p.render_obstacles(hard, soft)
+        p.run_nturn(sc.start, n_cycles)
+        try:
+            state["plan"] = p.extract_path(state["goal"])          # synchronises; plan comes back to the host
+        except nhp.NhpError as e:
+            if e.code != -5:
+                raise
+            state["plan"] = ([], 0xFFFFFFFF)
+
+    # warm-up, then choose a goal the sweeps actually reach (fixed for all timed steps)
+    for _ in range(max(args.warmup, 1)):
+        step(hard_d, soft_d)
+    p.status()
+    state["goal"] = pick_goal(p, sc, torch)
+    step(hard_d, soft_d)
+
+    def timed(hard, soft, profile):
+        p.kernel_times(reset=True)
+        p.set_profiling(profile)
+        l0 = p.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        replicas.barrier(); torch.cuda.synchronize()
+        e0.record()
+        for _ in range(args.steps):
+            step(hard, soft)
+        e1.record()
+        torch.cuda.synchronize(); replicas.barrier()
+        p.set_profiling(False)
+        return e0.elapsed_time(e1), p.launch_count() - l0
+
+    clocks = ClockSampler(local_rank)
+    if rank == 0:
+        clocks.start()
+    ms_dev, launches = timed(hard_d, soft_d, True)
+    kt = p.kernel_times(reset=True)
+    clk = clocks.stop() if rank == 0 else None
+    ms_e2e, _ = timed(hard_h, soft_h, False)
+    plan, cost = state["plan"]
+    ms_dev_max, units = replicas.aggregate(ms_dev, args.steps * updates_per_plan, dev)
+    ms_e2e_max, _ = replicas.aggregate(ms_e2e, 0, dev)
+    if rank != 0:
+        p.close(); replicas.shutdown()
+        return
+
+    peak, peak_src = peak_hbm()
+    alg_b = ALG_BYTES_SOFT if sc.soft is not None else ALG_BYTES_HARD
+    sweeps = {k: v for k, v in kt.items() if k in nhp.MANEUVER_NAMES or k == "fused"}
+    dom = max(sweeps, key=lambda k: sweeps[k][0])
+    dom_ms, dom_n = sweeps[dom]
+    per_launch_bytes = alg_b * n_r * (1 if dom != "fused" else 6)
+    achieved = per_launch_bytes / (dom_ms / max(dom_n, 1) * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+    sweep_ms = sum(v[0] for v in sweeps.values())
+    sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
+    out = {
+        "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config,
+                   "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)",
+                   "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
+                   "goal": list(state["goal"]), "plan_waypoints": len(plan), "plan_cost": cost},
+        "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
+        "clocks": clk,
+        "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
+                "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if soft_h is not None else 0)),
+                "d2h_bytes_per_step": int(16 * 4096 + 32)},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
+                     "launches_timed": int(dom_n),
+                     "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
+        "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
+    }
+    if not args.no_cpu_baseline and ws == 1:
+        out["cpu_baseline"] = cpu_baseline(sc, n_cycles, sample_cycles=2)
+    p.close()
+    replicas.shutdown()
+    print(json.dumps(out), flush=True)
+
+
+def oracle_setup(sc):
+    """Oracle handle plus its own rendering of the scene (the oracle never sees anything from the CUDA path)."""
+    import oracle
+    o = oracle.Oracle(sc.log2_n, sc.log2_nt, sc.R, sc.ct, sc.dir_mult, sc.cost_one_log2, sc.flags, threads=0)
+    fp = oracle.Footprint(sc.mask, sc.ou, sc.ov)
+    t0 = time.perf_counter()
+    Cv, Sv = o.render(fp, sc.hard, sc.soft, method="runs")
+    return o, Cv, Sv, time.perf_counter() - t0
+
+
+def cpu_baseline(sc, n_cycles, sample_cycles=2):
+    """The oracle as it stands on this box's host cores, on a bounded sample of the same workload: its own
+    rendering of the scene plus `sample_cycles` of the N_T maneuver cycles over the full volume.  The value is
+    plan-equivalent: sampled pose-updates / (sweep time + render time * sample_cycles / N_T)."""
+    import numpy as np
+    o, Cv, Sv, t_render = oracle_setup(sc)
+    V = np.full(o.shape, 0xFFFFFFFF, np.uint32)
+    V[sc.start[2], sc.start[1], sc.start[0]] = 0
+    t0 = time.perf_counter()
+    o.cycles(V, Cv, Sv, sample_cycles)
+    t_sweeps = time.perf_counter() - t0
+    upd = 6 * sample_cycles * V.size
+    return {"value": upd / (t_sweeps + t_render * sample_cycles / n_cycles) / 1e9, "unit": UNIT, "cores": int(o.threads),
+            "kind": "oracle",
+            "sample": f"oracle render of the full scene ({t_render:.2f} s) + {sample_cycles} of {n_cycles} maneuver cycles "
+                      f"over the full {sc.n}x{sc.n}x{sc.nt} volume ({t_sweeps:.2f} s), OpenMP over curves on all host cores; "
+                      f"render time charged pro rata"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (the only 'reference' this tier has), one bounded sample per step."""
+    from paper_2306_01301_b200 import replicas
+    rank, _, ws = replicas.world()
+    if rank != 0:
+        return
+    import numpy as np
+
+    import scenes
+    sc = scenes.get_config(args.config)
+    n_cycles = args.cycles or sc.n_cycles
+    o, Cv, Sv, t_render = oracle_setup(sc)
+    V = np.full(o.shape, 0xFFFFFFFF, np.uint32)
+    V[sc.start[2], sc.start[1], sc.start[0]] = 0
+    whole_cycle = (args.steps + args.warmup) <= 12
+    fwd_only = bool(sc.flags & 1)
+
+    def step(k):
+        if whole_cycle:
+            o.cycles(V, Cv, Sv, 1)
+            return (3 if fwd_only else 6) * V.size
+        o.sweep(k % 6, V, Cv, Sv)
+        return V.size
+
+    for k in range(args.warmup):
+        step(k)
+    t0 = time.perf_counter()
+    upd = sum(step(args.warmup + k) for k in range(args.steps))
+    dt = time.perf_counter() - t0
+    val = upd / dt / 1e9
+    sample = (("one maneuver cycle (6 sweeps)" if whole_cycle else "one maneuver sweep (maneuver = step mod 6)") +
+              f" over the full {sc.n}x{sc.n}x{sc.nt} volume per step; scene rendered once by the oracle before timing "
+              f"({t_render:.2f} s, not in the value)")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": ws, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": int(o.threads), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -175,6 +175,18 @@ int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t
 /* Number of kernels launched by this handle since creation (for bench.py's gpu_launches). */
 long long nhp_launch_count(const nhp_planner *p);
 
+/* Per-kernel device timing for bench.py's roofline line.  With profiling enabled every kernel launch of the
+ * handle is bracketed by a cudaEvent pair recorded on the handle's stream (up to 1024 launches between two
+ * reads; further launches run untimed).  nhp_kernel_times synchronises the stream, adds the elapsed times
+ * of the pairs recorded since the last read to running sums, copies the sums to HOST arrays of
+ * NHP_KERNEL_SLOTS entries and, with reset != 0, zeroes them.
+ *   slots 0..5  maneuver kernels in cycle order (LF, SF, RB, RF, SB, LB)
+ *   slot 6      collision rendering (a1), slot 7 soft rendering (a2), slot 8 volume init / export (a6),
+ *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing, slot 11 fused sweeps */
+#define NHP_KERNEL_SLOTS 12
+int nhp_set_profiling(nhp_planner *p, int enable);
+int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
+
 #ifdef __cplusplus
 }
 #endif

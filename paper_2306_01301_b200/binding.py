@@ -18,7 +18,10 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
            "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_run_nturn", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
-           "nhp_debug_tables", "nhp_launch_count")
+           "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
+KERNEL_SLOTS = 12
+KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
+                     "backtrack", "raster_pack", "fused")
 
 
 class Weights(C.Structure):
@@ -77,6 +80,8 @@ def load_library():
         L.nhp_debug_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.nhp_launch_count.argtypes = [C.c_void_p]
         L.nhp_launch_count.restype = C.c_longlong
+        L.nhp_set_profiling.argtypes = [C.c_void_p, C.c_int]
+        L.nhp_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
         _lib = L
     return _lib
 
@@ -205,6 +210,16 @@ class Planner:
 
     def launch_count(self):
         return int(self._L.nhp_launch_count(self._h))
+
+    def set_profiling(self, enable=True):
+        self._check(self._L.nhp_set_profiling(self._h, int(bool(enable))), "set_profiling")
+
+    def kernel_times(self, reset=False):
+        """-> {slot name: (summed ms, launches)} of the event-bracketed launches since the last reset."""
+        ms = (C.c_double * KERNEL_SLOTS)()
+        cnt = (C.c_longlong * KERNEL_SLOTS)()
+        self._check(self._L.nhp_kernel_times(self._h, ms, cnt, int(bool(reset))), "kernel_times")
+        return {KERNEL_SLOT_NAMES[k]: (ms[k], cnt[k]) for k in range(KERNEL_SLOTS)}
 
     # ---- host copies for tests ---------------------------------------------------------------
     def cost_volume_numpy(self):

@@ -171,6 +171,7 @@ int nhp_planner_destroy(nhp_planner *p)
     cudaFree(p->d_status); cudaFree(p->d_plan);
     if (p->h_status) cudaFreeHost(p->h_status);
     if (p->h_plan) cudaFreeHost(p->h_plan);
+    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     delete p;
     return NHP_OK;
 }
@@ -321,5 +322,36 @@ int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t
 }
 
 long long nhp_launch_count(const nhp_planner *p) { return p ? p->launches : 0; }
+
+int nhp_set_profiling(nhp_planner *p, int enable)
+{
+    if (!p) return NHP_E_ARG;
+    if (enable && p->ev.empty()) {
+        p->ev.resize(2 * PROF_PAIRS);
+        p->ev_slot.assign(PROF_PAIRS, 0);
+        for (auto &e : p->ev) CU(cudaEventCreate(&e));
+    }
+    p->profiling = enable != 0;
+    return NHP_OK;
+}
+
+int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset)
+{
+    if (!p) return NHP_E_ARG;
+    CU(cudaStreamSynchronize(p->stream));
+    for (int k = 0; k < p->ev_used; k++) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, p->ev[2 * k], p->ev[2 * k + 1]));
+        p->k_ms[p->ev_slot[k]] += ms;
+        p->k_launches[p->ev_slot[k]] += 1;
+    }
+    p->ev_used = 0;
+    for (int s = 0; s < NHP_KERNEL_SLOTS; s++) {
+        if (ms_sum) ms_sum[s] = p->k_ms[s];
+        if (launches) launches[s] = p->k_launches[s];
+        if (reset) { p->k_ms[s] = 0; p->k_launches[s] = 0; }
+    }
+    return NHP_OK;
+}
 
 }  // extern "C"

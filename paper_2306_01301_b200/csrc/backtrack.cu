@@ -163,6 +163,7 @@ int launch_backtrack(nhp_planner *p, int gi, int gj, int gt)
     P.si = p->start[0]; P.sj = p->start[1]; P.st = p->start[2];
     P.gi = gi; P.gj = gj; P.gt = gt;
     P.cap = p->plan_cap;
+    ProfScope prof(p, 9);
     backtrack_kernel<<<1, 192, 0, p->stream>>>(p->V, p->S, p->tables(), P, p->d_plan, p->d_status);
     return 1;
 }

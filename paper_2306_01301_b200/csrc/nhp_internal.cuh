@@ -62,8 +62,34 @@ struct nhp_planner {
     nhp_waypoint *h_plan = nullptr;
     std::string err = "ok";
     long long launches = 0;
+    // per-kernel timing (nhp_set_profiling): event pairs on the launching stream, drained at sync points
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;   // 2 * PROF_PAIRS events, created on first enable
+    std::vector<int> ev_slot;      // slot of each used pair
+    int ev_used = 0;
+    double k_ms[NHP_KERNEL_SLOTS] = {0};
+    long long k_launches[NHP_KERNEL_SLOTS] = {0};
 
     DevTables tables() const { return DevTables{d_beta, d_B, d_lenq, d_IJ}; }
+};
+
+constexpr int PROF_PAIRS = 1024;
+
+// Bracket one kernel launch (or one group of launches) with an event pair when profiling is on.
+struct ProfScope {
+    nhp_planner *p;
+    int pair;
+    ProfScope(nhp_planner *p_, int slot) : p(p_), pair(-1)
+    {
+        if (!p->profiling || p->ev_used >= PROF_PAIRS) return;
+        pair = p->ev_used++;
+        p->ev_slot[pair] = slot;
+        cudaEventRecord(p->ev[2 * pair], p->stream);
+    }
+    ~ProfScope()
+    {
+        if (pair >= 0) cudaEventRecord(p->ev[2 * pair + 1], p->stream);
+    }
 };
 
 // ---- kernel launchers (each returns the number of kernels it launched) ---------------------------

@@ -29,6 +29,7 @@ __global__ void footprint_raster_kernel(uint32_t *__restrict__ E, const uint8_t 
 int launch_footprint_raster(nhp_planner *p, int mw, int mh, int64_t ouq, int64_t ovq)
 {
     dim3 grid(p->sidew, p->side, p->nt), block(32);
+    ProfScope prof(p, 10);
     footprint_raster_kernel<<<grid, block, 0, p->stream>>>(p->d_E, p->d_mask, mw, mh, ouq, ovq, p->d_rot, p->rad,
                                                           p->side, p->sidew);
     return 1;
@@ -130,16 +131,21 @@ __global__ void __launch_bounds__(256) render_soft_kernel(uint8_t *__restrict__ 
             }
         }
     }
-    *(uint32_t *)(S + ((size_t)t * n + (j0 + ty)) * n + i0 + tx * 4) = acc;
+    if (i0 + tx * 4 < n)                                     // n = 32: the 64-wide tile wraps onto itself
+        *(uint32_t *)(S + ((size_t)t * n + (j0 + ty)) * n + i0 + tx * 4) = acc;
 }
 
 int launch_render(nhp_planner *p, bool soft)
 {
     const int n = p->n;
-    pack_hard_kernel<<<dim3(n / 32, n), 32, 0, p->stream>>>(p->d_H, p->d_hard, n);
+    {
+        ProfScope prof(p, 10);
+        pack_hard_kernel<<<dim3(n / 32, n), 32, 0, p->stream>>>(p->d_H, p->d_hard, n);
+    }
     int launches = 1;
     {
         constexpr int RJ = 16;
+        ProfScope prof(p, 6);
         const size_t smem = sizeof(uint32_t) * ((size_t)p->side * p->sidew + (size_t)(RJ + 2 * p->rad) * (n / 32));
         cudaFuncSetAttribute(render_collision_kernel<RJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         render_collision_kernel<RJ><<<dim3(n / RJ, p->nt), 256, smem, p->stream>>>(p->C, p->d_H, p->d_E, n, p->rad,
@@ -150,7 +156,8 @@ int launch_render(nhp_planner *p, bool soft)
         const int pw = ((STX + 2 * p->rad + 6) >> 2) + 1, ph = STY + 2 * p->rad;
         const size_t smem = sizeof(uint32_t) * ((size_t)p->side * p->sidew + (size_t)ph * pw);
         cudaFuncSetAttribute(render_soft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        render_soft_kernel<<<dim3(n / STX, n / STY, p->nt), 256, smem, p->stream>>>(p->S, p->d_soft, p->d_E, n,
+        ProfScope prof(p, 7);
+        render_soft_kernel<<<dim3(n < STX ? 1 : n / STX, n / STY, p->nt), 256, smem, p->stream>>>(p->S, p->d_soft, p->d_E, n,
                                                                                    p->rad, p->side, p->sidew);
         launches++;
     }

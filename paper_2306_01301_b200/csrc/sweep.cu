@@ -67,6 +67,7 @@ int launch_init_volume(nhp_planner *p, int si, int sj, int st)
 {
     const size_t nr = (size_t)p->n * p->n * p->nt, nq = nr / 4;
     const size_t sidx = ((size_t)st * p->n + sj) * p->n + si;
+    ProfScope prof(p, 8);
     init_volume_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, p->stream>>>((uint4 *)p->V, p->C, nq, sidx, p->d_status);
     return 1;
 }
@@ -74,6 +75,7 @@ int launch_init_volume(nhp_planner *p, int si, int sj, int st)
 int launch_export_volume(nhp_planner *p, bool to_canonical)
 {
     const size_t nr = (size_t)p->n * p->n * p->nt, nq = nr / 4;
+    ProfScope prof(p, 8);
     export_volume_kernel<<<(unsigned)((nq + 255) / 256), 256, 0, p->stream>>>((uint4 *)p->V, p->C, nq, to_canonical ? 1 : 0);
     return 1;
 }
@@ -141,6 +143,7 @@ static int launch_maneuver_simple(nhp_planner *p, int m)
     const uint32_t *lenq = p->d_lenq + (size_t)m * nt;
     const uint32_t ct = p->w.ct[m];
     const int threads = n < 128 ? n : 128;
+    ProfScope prof(p, m);
     if (m == M_SF || m == M_SB) {
         dim3 grid(n / threads, nt);
         if (soft)
