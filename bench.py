@@ -184,10 +184,11 @@ def run_ours(args):
 
     peak, peak_src = peak_hbm()
     alg_b = ALG_BYTES_SOFT if sc.soft is not None else ALG_BYTES_HARD
-    sweeps = {k: v for k, v in kt.items() if k in nhp.MANEUVER_NAMES or k == "fused"}
+    # sweep kernels by slot: a single maneuver per launch (N_R pose-updates), or a turn pair (RB+RF / LB+LF: 2 N_R)
+    sweeps = {k: v for k, v in kt.items() if (k in nhp.MANEUVER_NAMES or k == "turn_pair") and v[1]}
     dom = max(sweeps, key=lambda k: sweeps[k][0])
     dom_ms, dom_n = sweeps[dom]
-    per_launch_bytes = alg_b * n_r * (1 if dom != "fused" else 6)
+    per_launch_bytes = alg_b * n_r * (2 if dom == "turn_pair" else 1)
     achieved = per_launch_bytes / (dom_ms / max(dom_n, 1) * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
@@ -205,7 +206,7 @@ def run_ours(args):
                 "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if soft_h is not None else 0)),
                 "d2h_bytes_per_step": int(16 * 4096 + 32)},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+        "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": n_r * (2 if dom == "turn_pair" else 1), "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
                      "launches_timed": int(dom_n),

@@ -182,7 +182,8 @@ long long nhp_launch_count(const nhp_planner *p);
  * NHP_KERNEL_SLOTS entries and, with reset != 0, zeroes them.
  *   slots 0..5  maneuver kernels in cycle order (LF, SF, RB, RF, SB, LB)
  *   slot 6      collision rendering (a1), slot 7 soft rendering (a2), slot 8 volume init / export (a6),
- *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing, slot 11 fused sweeps */
+ *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing,
+ *   slot 11     turn-pair launches (RB+RF or LB+next LF in one kernel: two maneuvers per launch) */
 #define NHP_KERNEL_SLOTS 12
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);

@@ -21,7 +21,7 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
 KERNEL_SLOTS = 12
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
-                     "backtrack", "raster_pack", "fused")
+                     "backtrack", "raster_pack", "turn_pair")
 
 
 class Weights(C.Structure):

@@ -164,15 +164,184 @@ static int launch_maneuver_simple(nhp_planner *p, int m)
     return 1;
 }
 
-// Cycle driver, PAPER.md:392 + l.475.  FORWARD_ONLY keeps LF, SF, RF.
+// ---------------------------------------------------------------------------------------------
+// Turn sweeps, B200 version: a tile of 32 curves stays ON CHIP for both laps and, where the cycle order puts two
+// opposite-direction maneuvers of the same curve family next to each other (RB -> RF, LB -> next cycle's LF,
+// PAPER.md:475), for both maneuvers: one read of the volume serves four laps.
+//
+// Tile = 32 consecutive x' at one y' (eq (18): every Theta plane of the tile is one 128-byte row segment, shifted
+// by beta).  The N_theta planes are cut into S = N_theta / L sections (the paper's "Sections", appendix D,
+// PAPER.md:903-952, here inside one CTA): warp s keeps planes [sL, sL+L) of its 32 curves in REGISTERS.
+//   pass 1  every warp sweeps its section from v = infinity and records (M, D): the value leaving the section
+//           and the summed edge cost across it (>= VI_BIG if a blocked vertex interrupts it) -- (Sv, Sd) of
+//           Insert 3, l.923-928
+//   ripple  carry into section s = fold of the other sections' (M, D) once around the closed curve, starting
+//           from section s itself (this is what the first of the paper's "two full loops" computes, l.356)
+//   pass 3  every warp sweeps its section again from that carry and updates its registers (Insert 5, l.946-949)
+// (min, saturating +) is associative (DESIGN R18), so the result is bit-identical to the sequential two laps.
+// Rows are written back only by threads whose section changed.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t D_CAP = 1u << 31;     // "a blocked vertex interrupts this section" as a summed edge cost
+
+// One vertex of a sweep with the arriving value v (Insert 5).  The additions sit on the
+// dependency chain (a = v + w, then min(u + ct + w, a)) so that no per-vertex temporary outlives its step.
+__device__ __forceinline__ uint32_t chain_step(uint32_t v, uint32_t u, uint32_t w, uint32_t ctw)
+{
+    const uint32_t a = v + w;
+    return (u != 0u) ? __viaddmin_u32(u, ctw, a) : VI_BIG;
+}
+
+template <int L, bool UP>
+__device__ __forceinline__ uint32_t section_summary(const uint32_t (&col)[L], uint32_t w, uint32_t ctw)
+{
+    uint32_t v = VI_INF;
+#pragma unroll
+    for (int s = 0; s < L; s++) v = chain_step(v, col[UP ? s : L - 1 - s], w, ctw);
+    return v;
+}
+
+// Apply pass.  out = min(v, u) is what the vertex keeps; the value that travels on is
+// min(v + w, u + ct + w) = min(v + w, out + ct + w) (ct >= 0), written with `out` so that the stored value sits on
+// the dependency chain: the scheduler then cannot postpone it and keep every intermediate v alive in a register.
+template <int L, bool UP>
+__device__ __forceinline__ void section_apply(uint32_t (&col)[L], uint32_t w, uint32_t ctw, uint32_t v, bool &changed)
+{
+#pragma unroll
+    for (int s = 0; s < L; s++) {
+        const int k = UP ? s : L - 1 - s;
+        const uint32_t u = col[k];
+        const uint32_t out = min(v, u);
+        changed |= (v < u);                    // accumulates in a predicate: no register, no longer live range
+        col[k] = out;
+        v = chain_step(v, out, w, ctw);
+    }
+}
+
+// carry into section `sec` of a closed curve cut into S (a power of two) sections, travel direction UP
+// (sec -> sec+1) or down: fold the other sections once around the curve, starting from section sec itself.
+template <bool UP>
+__device__ __forceinline__ uint32_t ripple_carry(const uint32_t *sM, const uint32_t *sD, int sec, int S, int lane)
+{
+    uint32_t c = sM[sec * 32 + lane];
+#pragma unroll 1
+    for (int r = 1; r < S; r++) {
+        const int q = (UP ? sec + r : sec - r) & (S - 1);
+        c = __viaddmin_u32(c, sD[q * 32 + lane], sM[q * 32 + lane]);
+    }
+    return c;
+}
+
+struct TurnPass { uint32_t w, ctw; };
+
+template <int L, int NPASS, bool UP0>
+__global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const int16_t *__restrict__ beta,
+                                                          int log2_n, int nt, int qa, int qb, TurnPass pa, TurnPass pb)
+{
+    extern __shared__ uint32_t smem[];
+    const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
+    uint2 *soff = (uint2 *)smem;                              // [nt] (row base index, first column) of the tile
+    uint32_t *sM = smem + 2 * nt, *sD = sM + 2 * S * 32;      // [2][S][32] each
+    const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
+    const int x0 = blockIdx.x << 5, yp = blockIdx.y;
+    for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
+        soff[t] = make_uint2((uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n)), (uint32_t)((x0 + ba) & mx));
+    }
+    __syncthreads();
+    // keep the four weights in registers (otherwise they are re-fetched from the constant bank at every step)
+    uint32_t wa = pa.w, ctwa = pa.ctw, wb = pb.w, ctwb = pb.ctw;
+    asm volatile("" : "+r"(wa), "+r"(ctwa), "+r"(wb), "+r"(ctwb));
+    uint32_t col[L];
+#pragma unroll
+    for (int k = 0; k < L; k++) {
+        const uint2 o = soff[sec * L + k];
+        col[k] = V[o.x + ((o.y + lane) & mx)];
+    }
+    // blocked vertices never change, so "does a blocked vertex interrupt my section" is decided once
+    uint32_t lowest = col[0];
+#pragma unroll
+    for (int k = 1; k < L; k++) lowest = min(lowest, col[k]);
+    const bool interrupted = (lowest == 0u);
+    bool changed = false;
+    sM[sec * 32 + lane] = section_summary<L, UP0>(col, wa, ctwa);
+    sD[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wa;
+    __syncthreads();
+    section_apply<L, UP0>(col, wa, ctwa, ripple_carry<UP0>(sM, sD, sec, S, lane), changed);
+    if (NPASS == 2) {
+        uint32_t *sM2 = sM + S * 32, *sD2 = sD + S * 32;
+        sM2[sec * 32 + lane] = section_summary<L, !UP0>(col, wb, ctwb);
+        sD2[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wb;
+        __syncthreads();
+        section_apply<L, !UP0>(col, wb, ctwb, ripple_carry<!UP0>(sM2, sD2, sec, S, lane), changed);
+    }
+    if (changed) {
+        int row0 = sec * L;
+        asm volatile("" : "+r"(row0));        // recompute the addresses: keeping 64 of them alive across the passes spills
+#pragma unroll
+        for (int k = 0; k < L; k++) {
+            const uint2 o = soff[row0 + k];
+            V[o.x + ((o.y + lane) & mx)] = col[k];
+        }
+    }
+}
+
+// Can the tile kernel serve this planner?  Needs N_theta = 32 S with S <= 32 (one CTA) and 32-bit element indices.
+static int turn_tile_L(const nhp_planner *p)
+{
+    if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
+    if (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) return 0;            // soft variant: simple kernels for now
+    if ((size_t)p->n * p->n * p->nt > ((size_t)1 << 32)) return 0;
+    return p->nt <= 1024 ? 32 : 0;
+}
+
+// One launch = maneuver ma (and then mb, the opposite direction on the same curve family, if mb >= 0).
+static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
+{
+    const int n = p->n, nt = p->nt, S = nt / L;
+    const bool left = (ma == M_LF || ma == M_LB);
+    const int qa = left ? 0 : 2, qb = left ? 3 : 1;
+    const bool up = (ma == M_LF || ma == M_RB);
+    auto pass = [&](int m) {
+        TurnPass t{0, 0};
+        if (m >= 0) { t.w = p->len_q[(size_t)m * nt]; t.ctw = p->w.ct[m] + t.w; }       // turn edge length does not depend on Theta (l.334)
+        return t;
+    };
+    const TurnPass pa = pass(ma), pb = pass(mb);
+    const dim3 grid(n / 32, n), block(32 * S);
+    const size_t smem = sizeof(uint32_t) * (2 * (size_t)nt + 4 * (size_t)S * 32);
+    ProfScope prof(p, mb >= 0 ? 11 : ma);
+#define NHP_TT(LL, NP, UP) turn_tile_kernel<LL, NP, UP><<<grid, block, smem, p->stream>>>(p->V, p->d_beta, p->log2_n, nt, qa, qb, pa, pb)
+    if (mb >= 0) { if (up) NHP_TT(32, 2, true); else NHP_TT(32, 2, false); }
+    else { if (up) NHP_TT(32, 1, true); else NHP_TT(32, 1, false); }
+#undef NHP_TT
+    return 1;
+}
+
+// Cycle driver, PAPER.md:392 + l.475: LF, SF, RB, RF, SB, LB per cycle.  FORWARD_ONLY keeps LF, SF, RF.
+// With the tile kernel, RB+RF run as one launch and LB is fused with the LF of the NEXT cycle (same curve family,
+// adjacent in the sequence), so the order of operations on every vertex is exactly the paper's.
 int launch_cycles(nhp_planner *p, int n_cycles)
 {
     int launches = 0;
     const bool fwd_only = p->w.flags & NHP_FLAG_FORWARD_ONLY;
-    for (int c = 0; c < n_cycles; c++)
-        for (int m = 0; m < 6; m++) {
-            if (fwd_only && (m == M_RB || m == M_SB || m == M_LB)) continue;
-            launches += launch_maneuver_simple(p, m);
+    const int L = turn_tile_L(p);
+    for (int c = 0; c < n_cycles; c++) {
+        if (L == 0) {
+            for (int m = 0; m < 6; m++) {
+                if (fwd_only && (m == M_RB || m == M_SB || m == M_LB)) continue;
+                launches += launch_maneuver_simple(p, m);
+            }
+        } else if (fwd_only) {
+            launches += launch_turn_tile(p, L, M_LF, -1);
+            launches += launch_maneuver_simple(p, M_SF);
+            launches += launch_turn_tile(p, L, M_RF, -1);
+        } else {
+            if (c == 0) launches += launch_turn_tile(p, L, M_LF, -1);
+            launches += launch_maneuver_simple(p, M_SF);
+            launches += launch_turn_tile(p, L, M_RB, M_RF);
+            launches += launch_maneuver_simple(p, M_SB);
+            launches += (c + 1 < n_cycles) ? launch_turn_tile(p, L, M_LB, M_LF) : launch_turn_tile(p, L, M_LB, -1);
         }
+    }
     return launches;
 }
