@@ -99,3 +99,4 @@ int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);
+int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable

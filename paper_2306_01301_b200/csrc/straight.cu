@@ -1,0 +1,213 @@
+// Straight sweeps SF / SB, B200 version.
+// PAPER.md:271-302 (section V.C, eqs (19)-(24): the discretised lines of one Theta slice), l.294 (direction by
+// J), l.356 (one lap, started at the wall), Insert 5 l.946-949 (loop body), l.366-370 (the coalescing problem the
+// paper solves with transposed slices and that is solved here by staging tiles in shared memory).
+//
+// One WARP owns a band of 32 neighbouring lines x' in [X0, X0+32) of one slice and walks along them in tiles of
+// 32 sweep steps, carrying the arriving value v of its 32 lines in registers (thread = line).  Tiles are brought
+// into shared memory by cp.async, ST_NBUF - 1 tiles ahead of the one being relaxed, so that the dependent chain
+// of a line never waits for HBM.  In shared memory element (line l, step k) of a tile sits at word l*33 + k:
+//   * slices with I = 0 (|tan| <= 1, eq (19)): step = i, j = (x' + B(i)) & mask, eq (23).  The tile is a
+//     parallelogram of the slice: rows r0 .. r0+31+span, 128-byte row segments, each lane (= column i) copying
+//     the 32 rows that belong to its column; the transposition to "thread = line" happens in the shared-memory
+//     addressing, both directions conflict-free (bank = l + k).
+//   * slices with I = 1: step = j, i = (x' + B(j)) & mask: every step is one (misaligned) 128-byte row segment.
+// A tile is written back (again as row segments) only if a value in it improved.
+#include "nhp_internal.cuh"
+
+namespace {
+
+constexpr int ST_NBUF = 3;                 // tiles in flight per warp (one being relaxed, two arriving)
+constexpr int ST_STRIDE = 33;              // words per line in a tile (padding -> conflict-free both ways)
+constexpr int ST_TILE_WORDS = 32 * ST_STRIDE;
+
+__device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void *gptr)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// Geometry of one tile of a band, as the load and the store phase need it (recomputed, never kept: 3 registers).
+struct TileGeo {
+    int delta;                 // class X: first row of this lane's column inside the parallelogram
+    int row0, rdir, nrows;     // class X: rows (row0 + rdir q) & mask, q < nrows <= 64
+    int bmine;                 // B(32 T + lane): class Y broadcasts it row by row
+};
+
+template <bool XCLASS>
+__device__ __forceinline__ TileGeo tile_geometry(const int16_t *__restrict__ Bt, int T, int X0, int lane, bool pos)
+{
+    TileGeo g;
+    g.bmine = Bt[32 * T + lane];
+    g.delta = 0; g.row0 = 0; g.rdir = 1; g.nrows = 32;
+    if (XCLASS) {
+        // B(i) is monotone in i, so its extremes over the tile sit in lanes 0 and 31
+        const int b0 = __shfl_sync(0xffffffffu, g.bmine, 0), b31 = __shfl_sync(0xffffffffu, g.bmine, 31);
+        const int bmin = min(b0, b31), bmax = max(b0, b31);
+        // rows are numbered so that delta is non-increasing in the lane index (conflict-free staging, see top)
+        g.delta = pos ? bmax - g.bmine : g.bmine - bmin;
+        g.row0 = pos ? X0 + bmax + 31 : X0 + bmin;
+        g.rdir = pos ? -1 : 1;
+        g.nrows = 32 + bmax - bmin;
+    }
+    return g;
+}
+
+// cp.async of tile T into `tile` (shared-memory byte address of the warp's buffer).  The row loops are unrolled
+// by 8 only: the whole kernel has to stay inside the instruction cache (a fully unrolled version ran at
+// "no instruction" stalls of 3-7 per issue, profiles/r01_tile_kernels.md).
+template <bool XCLASS>
+__device__ __forceinline__ void tile_load(uint32_t tile, const uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, int T,
+                                          int X0, int lane, int log2_n, bool pos)
+{
+    const int mx = (1 << log2_n) - 1;
+    const TileGeo g = tile_geometry<XCLASS>(Bt, T, X0, lane, pos);
+    if (XCLASS) {
+        // lane = column i = 32 T + lane; row q of the parallelogram goes to line (q - delta) of the tile
+        uint32_t sa = tile + 4u * (uint32_t)(lane - g.delta * ST_STRIDE);
+        const uint32_t *col = Vt + 32 * T + lane;
+        unsigned long long act = 0xffffffffull << g.delta;                      // bit q: my column owns row q
+        int r = g.row0;
+        for (int q0 = 0; q0 < g.nrows; q0 += 8) {                                // warp-uniform trip count
+#pragma unroll
+            for (int qq = 0; qq < 8; qq++) {
+                if (((uint32_t)act >> qq) & 1u) cp_async4(sa + 4u * (uint32_t)(qq * ST_STRIDE), col + ((size_t)(r & mx) << log2_n));
+                r += g.rdir;
+            }
+            act >>= 8;
+            sa += 4u * 8u * ST_STRIDE;
+        }
+    } else {
+        // step k = row j = 32 T + k; lane = line: column (X0 + B(j) + lane) & mask
+        const uint32_t sa = tile + 4u * (uint32_t)(lane * ST_STRIDE);
+        const uint32_t *row = Vt + ((size_t)(32 * T) << log2_n);
+#pragma unroll 8
+        for (int k = 0; k < 32; k++) {
+            const int b = __shfl_sync(0xffffffffu, g.bmine, k);
+            cp_async4(sa + 4u * (uint32_t)k, row + ((size_t)k << log2_n) + ((X0 + b + lane) & mx));
+        }
+    }
+}
+
+// write tile T back; cm = this thread's (= line's) mask of improved steps
+template <bool XCLASS>
+__device__ __forceinline__ void tile_store(const uint32_t *tile, uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, int T,
+                                           int X0, int lane, int log2_n, bool pos, uint32_t cm)
+{
+    const int mx = (1 << log2_n) - 1;
+    const TileGeo g = tile_geometry<XCLASS>(Bt, T, X0, lane, pos);
+    if (XCLASS) {
+        const uint32_t lines = __ballot_sync(0xffffffffu, cm != 0u);             // lines with an improved value
+        const uint32_t *sb = tile + (lane - g.delta * ST_STRIDE);
+        uint32_t *col = Vt + 32 * T + lane;
+        unsigned long long want = (unsigned long long)lines << g.delta;          // rows of my column on those lines
+        int r = g.row0;
+        for (int q0 = 0; q0 < g.nrows; q0 += 8) {
+#pragma unroll
+            for (int qq = 0; qq < 8; qq++) {
+                if (((uint32_t)want >> qq) & 1u) col[(size_t)(r & mx) << log2_n] = sb[qq * ST_STRIDE];
+                r += g.rdir;
+            }
+            want >>= 8;
+            sb += 8 * ST_STRIDE;
+        }
+    } else {
+        const uint32_t *sb = tile + lane * ST_STRIDE;
+        uint32_t *row = Vt + ((size_t)(32 * T) << log2_n);
+#pragma unroll 8
+        for (int k = 0; k < 32; k++) {
+            const int b = __shfl_sync(0xffffffffu, g.bmine, k);
+            if ((cm >> k) & 1u) row[((size_t)k << log2_n) + ((X0 + b + lane) & mx)] = sb[k];
+        }
+    }
+}
+
+// Relax the 32 steps of a tile for this thread's line (Insert 5, internal encoding):
+//   V[i] = min(v, u);  v = min(v, u + ct) + (blocked ? infinity : w)
+template <bool UP>
+__device__ __forceinline__ uint32_t tile_relax(uint32_t *line, uint32_t &v, uint32_t w, uint32_t ct)
+{
+    uint32_t cm = 0;
+#pragma unroll
+    for (int s = 0; s < 32; s++) {
+        const int k = UP ? s : 31 - s;
+        const uint32_t u = line[k];
+        if (v < u) { line[k] = v; cm |= 1u << k; }
+        v = __viaddmin_u32(u, ct, v) + (u != 0u ? w : VI_BIG);
+    }
+    return cm;
+}
+
+template <bool XCLASS>
+__device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, uint32_t *buf, int X0,
+                                           int lane, int log2_n, uint32_t w, uint32_t ct, bool pos, bool up)
+{
+    const int NT = 1 << (log2_n - 5);
+    const uint32_t sbuf = (uint32_t)__cvta_generic_to_shared(buf);
+    for (int s = 0; s < ST_NBUF - 1; s++) {
+        if (s < NT) tile_load<XCLASS>(sbuf + 4u * (uint32_t)(s * ST_TILE_WORDS), Vt, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos);
+        cp_async_commit();
+    }
+    uint32_t v = VI_INF;
+    int b = 0, bn = ST_NBUF - 1;                      // buffer of tile s, buffer of tile s + NBUF - 1
+#pragma unroll 1
+    for (int s = 0; s < NT; s++) {
+        cp_async_wait<ST_NBUF - 2>();
+        __syncwarp();
+        {   // prefetch tile s + NBUF - 1 into the buffer tile s - 1 has just left
+            const int sn = s + ST_NBUF - 1;
+            if (sn < NT) tile_load<XCLASS>(sbuf + 4u * (uint32_t)(bn * ST_TILE_WORDS), Vt, Bt, up ? sn : NT - 1 - sn, X0, lane, log2_n, pos);
+            cp_async_commit();
+        }
+        uint32_t *tile = buf + b * ST_TILE_WORDS;
+        const uint32_t cm = up ? tile_relax<true>(tile + lane * ST_STRIDE, v, w, ct) : tile_relax<false>(tile + lane * ST_STRIDE, v, w, ct);
+        if (__any_sync(0xffffffffu, cm != 0u)) {
+            __syncwarp();
+            tile_store<XCLASS>(tile, Vt, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos, cm);
+        }
+        b = (b + 1 == ST_NBUF) ? 0 : b + 1;
+        bn = (bn + 1 == ST_NBUF) ? 0 : bn + 1;
+    }
+}
+
+__global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict__ V, const int16_t *__restrict__ B,
+                                                            const uint8_t *__restrict__ IJ, const uint32_t *__restrict__ lenq,
+                                                            uint32_t ct, int log2_n, int is_forward)
+{
+    extern __shared__ uint32_t smem[];
+    const int n = 1 << log2_n, t = blockIdx.y;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
+    const int I = IJ[t] & 1, jpos = (IJ[t] >> 1) & 1;
+    const bool up = (is_forward == jpos);                                       // eq (24)
+    const int16_t *Bt = B + (size_t)t * n;
+    const bool pos = Bt[n - 1] >= 0;                                            // sign of K(Theta), eq (20)
+    uint32_t *Vt = V + ((size_t)t << (2 * log2_n));
+    uint32_t *buf = smem + warp * (ST_NBUF * ST_TILE_WORDS);
+    const uint32_t w = lenq[t];
+    if (I == 0) band_sweep<true>(Vt, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
+    else band_sweep<false>(Vt, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
+}
+
+}  // namespace
+
+// SF or SB over the whole volume; returns the number of kernels launched (0 = not applicable, use the simple kernel)
+int launch_straight_tile(nhp_planner *p, int m)
+{
+    if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
+    if (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) return 0;               // soft variant: simple kernels for now
+    const int n = p->n, nt = p->nt;
+    const int bands = n / 32, warps = bands < 4 ? bands : 4;
+    const size_t smem = sizeof(uint32_t) * (size_t)warps * ST_NBUF * ST_TILE_WORDS;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(straight_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * ST_NBUF * ST_TILE_WORDS * 4);
+        attr_set = true;
+    }
+    ProfScope prof(p, m);
+    straight_tile_kernel<<<dim3(bands / warps, nt), warps * 32, smem, p->stream>>>(p->V, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
+                                                                                   p->w.ct[m], p->log2_n, m == M_SF);
+    return 1;
+}

@@ -183,37 +183,34 @@ static int launch_maneuver_simple(nhp_planner *p, int m)
 // ---------------------------------------------------------------------------------------------
 constexpr uint32_t D_CAP = 1u << 31;     // "a blocked vertex interrupts this section" as a summed edge cost
 
-// One vertex of a sweep with the arriving value v (Insert 5).  The additions sit on the
-// dependency chain (a = v + w, then min(u + ct + w, a)) so that no per-vertex temporary outlives its step.
-__device__ __forceinline__ uint32_t chain_step(uint32_t v, uint32_t u, uint32_t w, uint32_t ctw)
+// One vertex of a sweep with the arriving value v, exactly the paper's line (Insert 5):
+//     v = min(v, u + ct) + cx * B[i]
+// with the edge weight "infinite" at a blocked vertex (u == 0).  One DPX instruction + one add on the chain.
+__device__ __forceinline__ uint32_t chain_step(uint32_t v, uint32_t u, uint32_t w, uint32_t ct)
 {
-    const uint32_t a = v + w;
-    return (u != 0u) ? __viaddmin_u32(u, ctw, a) : VI_BIG;
+    return __viaddmin_u32(u, ct, v) + (u != 0u ? w : VI_BIG);
 }
 
 template <int L, bool UP>
-__device__ __forceinline__ uint32_t section_summary(const uint32_t (&col)[L], uint32_t w, uint32_t ctw)
+__device__ __forceinline__ uint32_t section_summary(const uint32_t (&col)[L], uint32_t w, uint32_t ct)
 {
     uint32_t v = VI_INF;
 #pragma unroll
-    for (int s = 0; s < L; s++) v = chain_step(v, col[UP ? s : L - 1 - s], w, ctw);
+    for (int s = 0; s < L; s++) v = chain_step(v, col[UP ? s : L - 1 - s], w, ct);
     return v;
 }
 
-// Apply pass.  out = min(v, u) is what the vertex keeps; the value that travels on is
-// min(v + w, u + ct + w) = min(v + w, out + ct + w) (ct >= 0), written with `out` so that the stored value sits on
-// the dependency chain: the scheduler then cannot postpone it and keep every intermediate v alive in a register.
+// Apply pass: the vertex keeps min(v, u); the value that travels on is the same chain step.
 template <int L, bool UP>
-__device__ __forceinline__ void section_apply(uint32_t (&col)[L], uint32_t w, uint32_t ctw, uint32_t v, bool &changed)
+__device__ __forceinline__ void section_apply(uint32_t (&col)[L], uint32_t w, uint32_t ct, uint32_t v, bool &changed)
 {
 #pragma unroll
     for (int s = 0; s < L; s++) {
         const int k = UP ? s : L - 1 - s;
         const uint32_t u = col[k];
-        const uint32_t out = min(v, u);
         changed |= (v < u);                    // accumulates in a predicate: no register, no longer live range
-        col[k] = out;
-        v = chain_step(v, out, w, ctw);
+        col[k] = min(v, u);
+        v = chain_step(v, u, w, ct);
     }
 }
 
@@ -231,7 +228,7 @@ __device__ __forceinline__ uint32_t ripple_carry(const uint32_t *sM, const uint3
     return c;
 }
 
-struct TurnPass { uint32_t w, ctw; };
+struct TurnPass { uint32_t w, ct; };
 
 template <int L, int NPASS, bool UP0>
 __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const int16_t *__restrict__ beta,
@@ -248,9 +245,11 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         soff[t] = make_uint2((uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n)), (uint32_t)((x0 + ba) & mx));
     }
     __syncthreads();
-    // keep the four weights in registers (otherwise they are re-fetched from the constant bank at every step)
-    uint32_t wa = pa.w, ctwa = pa.ctw, wb = pb.w, ctwb = pb.ctw;
-    asm volatile("" : "+r"(wa), "+r"(ctwa), "+r"(wb), "+r"(ctwb));
+    // The apply passes take their weight through an opaque copy: otherwise the compiler keeps the 32 per-vertex
+    // edge weights of the summary pass alive for the apply pass (common sub-expression) and spills them.
+    const uint32_t wa = pa.w, ctwa = pa.ct, wb = pb.w, ctwb = pb.ct;
+    uint32_t wa2 = pa.w, wb2 = pb.w;
+    asm volatile("" : "+r"(wa2), "+r"(wb2));
     uint32_t col[L];
 #pragma unroll
     for (int k = 0; k < L; k++) {
@@ -266,13 +265,13 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     sM[sec * 32 + lane] = section_summary<L, UP0>(col, wa, ctwa);
     sD[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wa;
     __syncthreads();
-    section_apply<L, UP0>(col, wa, ctwa, ripple_carry<UP0>(sM, sD, sec, S, lane), changed);
+    section_apply<L, UP0>(col, wa2, ctwa, ripple_carry<UP0>(sM, sD, sec, S, lane), changed);
     if (NPASS == 2) {
         uint32_t *sM2 = sM + S * 32, *sD2 = sD + S * 32;
         sM2[sec * 32 + lane] = section_summary<L, !UP0>(col, wb, ctwb);
         sD2[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wb;
         __syncthreads();
-        section_apply<L, !UP0>(col, wb, ctwb, ripple_carry<!UP0>(sM2, sD2, sec, S, lane), changed);
+        section_apply<L, !UP0>(col, wb2, ctwb, ripple_carry<!UP0>(sM2, sD2, sec, S, lane), changed);
     }
     if (changed) {
         int row0 = sec * L;
@@ -303,7 +302,7 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     const bool up = (ma == M_LF || ma == M_RB);
     auto pass = [&](int m) {
         TurnPass t{0, 0};
-        if (m >= 0) { t.w = p->len_q[(size_t)m * nt]; t.ctw = p->w.ct[m] + t.w; }       // turn edge length does not depend on Theta (l.334)
+        if (m >= 0) { t.w = p->len_q[(size_t)m * nt]; t.ct = p->w.ct[m]; }       // turn edge length does not depend on Theta (l.334)
         return t;
     };
     const TurnPass pa = pass(ma), pb = pass(mb);
@@ -315,6 +314,12 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     else { if (up) NHP_TT(32, 1, true); else NHP_TT(32, 1, false); }
 #undef NHP_TT
     return 1;
+}
+
+static int launch_straight(nhp_planner *p, int m)
+{
+    const int k = launch_straight_tile(p, m);
+    return k ? k : launch_maneuver_simple(p, m);
 }
 
 // Cycle driver, PAPER.md:392 + l.475: LF, SF, RB, RF, SB, LB per cycle.  FORWARD_ONLY keeps LF, SF, RF.
@@ -329,17 +334,17 @@ int launch_cycles(nhp_planner *p, int n_cycles)
         if (L == 0) {
             for (int m = 0; m < 6; m++) {
                 if (fwd_only && (m == M_RB || m == M_SB || m == M_LB)) continue;
-                launches += launch_maneuver_simple(p, m);
+                launches += (m == M_SF || m == M_SB) ? launch_straight(p, m) : launch_maneuver_simple(p, m);
             }
         } else if (fwd_only) {
             launches += launch_turn_tile(p, L, M_LF, -1);
-            launches += launch_maneuver_simple(p, M_SF);
+            launches += launch_straight(p, M_SF);
             launches += launch_turn_tile(p, L, M_RF, -1);
         } else {
             if (c == 0) launches += launch_turn_tile(p, L, M_LF, -1);
-            launches += launch_maneuver_simple(p, M_SF);
+            launches += launch_straight(p, M_SF);
             launches += launch_turn_tile(p, L, M_RB, M_RF);
-            launches += launch_maneuver_simple(p, M_SB);
+            launches += launch_straight(p, M_SB);
             launches += (c + 1 < n_cycles) ? launch_turn_tile(p, L, M_LB, M_LF) : launch_turn_tile(p, L, M_LB, -1);
         }
     }
