@@ -21,9 +21,16 @@ constexpr int ST_NBUF = 3;                 // tiles in flight per warp (one bein
 constexpr int ST_STRIDE = 33;              // words per line in a tile (padding -> conflict-free both ways)
 constexpr int ST_TILE_WORDS = 32 * ST_STRIDE;
 
-__device__ __forceinline__ void cp_async4(uint32_t smem_addr, const void *gptr)
+// Global addresses are formed as (opaque 64-bit slice base) + 4 * (32-bit element offset): one IMAD.WIDE.  The base
+// is made opaque once per warp so that the compiler keeps it in a register pair instead of re-deriving it from
+// the kernel parameters at every row.
+__device__ __forceinline__ void cp_async4(uint32_t smem_addr, unsigned long long vbase, uint32_t off)
 {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(smem_addr), "l"(gptr) : "memory");
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(smem_addr), "l"(vbase + 4ull * off) : "memory");
+}
+__device__ __forceinline__ void st_global(unsigned long long vbase, uint32_t off, uint32_t val)
+{
+    asm volatile("st.global.u32 [%0], %1;\n" ::"l"(vbase + 4ull * off), "r"(val) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
@@ -59,7 +66,7 @@ __device__ __forceinline__ TileGeo tile_geometry(const int16_t *__restrict__ Bt,
 // by 8 only: the whole kernel has to stay inside the instruction cache (a fully unrolled version ran at
 // "no instruction" stalls of 3-7 per issue, profiles/r01_tile_kernels.md).
 template <bool XCLASS>
-__device__ __forceinline__ void tile_load(uint32_t tile, const uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, int T,
+__device__ __forceinline__ void tile_load(uint32_t tile, unsigned long long Vt, const int16_t *__restrict__ Bt, int T,
                                           int X0, int lane, int log2_n, bool pos)
 {
     const int mx = (1 << log2_n) - 1;
@@ -67,14 +74,15 @@ __device__ __forceinline__ void tile_load(uint32_t tile, const uint32_t *__restr
     if (XCLASS) {
         // lane = column i = 32 T + lane; row q of the parallelogram goes to line (q - delta) of the tile
         uint32_t sa = tile + 4u * (uint32_t)(lane - g.delta * ST_STRIDE);
-        const uint32_t *col = Vt + 32 * T + lane;
         unsigned long long act = 0xffffffffull << g.delta;                      // bit q: my column owns row q
-        int r = g.row0;
+        // element offset inside the slice; "& smask" wraps the row index (the slice is a torus)
+        const uint32_t smask = (1u << (2 * log2_n)) - 1u, rstep = (uint32_t)(g.rdir << log2_n);
+        uint32_t off = (((uint32_t)g.row0 << log2_n) + (uint32_t)(32 * T + lane)) & smask;
         for (int q0 = 0; q0 < g.nrows; q0 += 8) {                                // warp-uniform trip count
 #pragma unroll
             for (int qq = 0; qq < 8; qq++) {
-                if (((uint32_t)act >> qq) & 1u) cp_async4(sa + 4u * (uint32_t)(qq * ST_STRIDE), col + ((size_t)(r & mx) << log2_n));
-                r += g.rdir;
+                if (((uint32_t)act >> qq) & 1u) cp_async4(sa + 4u * (uint32_t)(qq * ST_STRIDE), Vt, off);
+                off = (off + rstep) & smask;
             }
             act >>= 8;
             sa += 4u * 8u * ST_STRIDE;
@@ -82,18 +90,20 @@ __device__ __forceinline__ void tile_load(uint32_t tile, const uint32_t *__restr
     } else {
         // step k = row j = 32 T + k; lane = line: column (X0 + B(j) + lane) & mask
         const uint32_t sa = tile + 4u * (uint32_t)(lane * ST_STRIDE);
-        const uint32_t *row = Vt + ((size_t)(32 * T) << log2_n);
+        const uint32_t c0 = (uint32_t)(X0 + lane), n = 1u << log2_n;
+        uint32_t rowoff = (uint32_t)(32 * T) << log2_n;
 #pragma unroll 8
         for (int k = 0; k < 32; k++) {
             const int b = __shfl_sync(0xffffffffu, g.bmine, k);
-            cp_async4(sa + 4u * (uint32_t)k, row + ((size_t)k << log2_n) + ((X0 + b + lane) & mx));
+            cp_async4(sa + 4u * (uint32_t)k, Vt, rowoff + ((c0 + (uint32_t)b) & (uint32_t)mx));
+            rowoff += n;
         }
     }
 }
 
 // write tile T back; cm = this thread's (= line's) mask of improved steps
 template <bool XCLASS>
-__device__ __forceinline__ void tile_store(const uint32_t *tile, uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, int T,
+__device__ __forceinline__ void tile_store(const uint32_t *tile, unsigned long long Vt, const int16_t *__restrict__ Bt, int T,
                                            int X0, int lane, int log2_n, bool pos, uint32_t cm)
 {
     const int mx = (1 << log2_n) - 1;
@@ -101,25 +111,27 @@ __device__ __forceinline__ void tile_store(const uint32_t *tile, uint32_t *__res
     if (XCLASS) {
         const uint32_t lines = __ballot_sync(0xffffffffu, cm != 0u);             // lines with an improved value
         const uint32_t *sb = tile + (lane - g.delta * ST_STRIDE);
-        uint32_t *col = Vt + 32 * T + lane;
         unsigned long long want = (unsigned long long)lines << g.delta;          // rows of my column on those lines
-        int r = g.row0;
+        const uint32_t smask = (1u << (2 * log2_n)) - 1u, rstep = (uint32_t)(g.rdir << log2_n);
+        uint32_t off = (((uint32_t)g.row0 << log2_n) + (uint32_t)(32 * T + lane)) & smask;
         for (int q0 = 0; q0 < g.nrows; q0 += 8) {
 #pragma unroll
             for (int qq = 0; qq < 8; qq++) {
-                if (((uint32_t)want >> qq) & 1u) col[(size_t)(r & mx) << log2_n] = sb[qq * ST_STRIDE];
-                r += g.rdir;
+                if (((uint32_t)want >> qq) & 1u) st_global(Vt, off, sb[qq * ST_STRIDE]);
+                off = (off + rstep) & smask;
             }
             want >>= 8;
             sb += 8 * ST_STRIDE;
         }
     } else {
         const uint32_t *sb = tile + lane * ST_STRIDE;
-        uint32_t *row = Vt + ((size_t)(32 * T) << log2_n);
+        const uint32_t c0 = (uint32_t)(X0 + lane), n = 1u << log2_n;
+        uint32_t rowoff = (uint32_t)(32 * T) << log2_n;
 #pragma unroll 8
         for (int k = 0; k < 32; k++) {
             const int b = __shfl_sync(0xffffffffu, g.bmine, k);
-            if ((cm >> k) & 1u) row[((size_t)k << log2_n) + ((X0 + b + lane) & mx)] = sb[k];
+            if ((cm >> k) & 1u) st_global(Vt, rowoff + ((c0 + (uint32_t)b) & (uint32_t)mx), sb[k]);
+            rowoff += n;
         }
     }
 }
@@ -141,10 +153,12 @@ __device__ __forceinline__ uint32_t tile_relax(uint32_t *line, uint32_t &v, uint
 }
 
 template <bool XCLASS>
-__device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vt, const int16_t *__restrict__ Bt, uint32_t *buf, int X0,
+__device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const int16_t *__restrict__ Bt, uint32_t *buf, int X0,
                                            int lane, int log2_n, uint32_t w, uint32_t ct, bool pos, bool up)
 {
     const int NT = 1 << (log2_n - 5);
+    unsigned long long Vt = (unsigned long long)Vslice;
+    asm volatile("" : "+l"(Vt));
     const uint32_t sbuf = (uint32_t)__cvta_generic_to_shared(buf);
     for (int s = 0; s < ST_NBUF - 1; s++) {
         if (s < NT) tile_load<XCLASS>(sbuf + 4u * (uint32_t)(s * ST_TILE_WORDS), Vt, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos);
