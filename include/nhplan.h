@@ -78,7 +78,8 @@ typedef struct nhp_sizes {
     size_t V_bytes;          /* value volume, uint32 per vertex            (one volume) */
     size_t C_bytes;          /* collision volume, 1 bit per vertex             */
     size_t S_bytes;          /* soft volume, uint8 per vertex; 0 without NHP_FLAG_SOFT  */
-    size_t workspace_bytes;  /* scratch; may be 0                                                       */
+    size_t workspace_bytes;  /* 3 N_R bytes with NHP_FLAG_SOFT (curve-major copies of S for the left-turn, right-turn
+                                and straight sweeps, written by nhp_render_obstacles), else 0                     */
 } nhp_sizes;
 
 /* Caller-owned DEVICE buffers (e.g. torch tensors), 256-byte aligned, alive until nhp_planner_destroy. */
@@ -86,7 +87,7 @@ typedef struct nhp_buffers {
     void *V;                 /* V_bytes */
     void *C;                 /* C_bytes: word (Theta*N + j)*N/32 + i/32, bit i%32 = vertex (i,j,Theta) collides */
     void *S;                 /* S_bytes or NULL: Q4.4 speed-reciprocal of vertex idx, >= 16 */
-    void *workspace;         /* workspace_bytes or NULL */
+    void *workspace;         /* workspace_bytes (required with NHP_FLAG_SOFT) or NULL */
 } nhp_buffers;
 
 /* One transition point of a plan ("plan"): the vertex and the maneuver that ARRIVES at it

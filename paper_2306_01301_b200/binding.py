@@ -113,9 +113,11 @@ class Planner:
             self.V = torch.empty(sz.V_bytes // 4, dtype=torch.int32, device=self.device)
             self.C = torch.empty(sz.C_bytes // 4, dtype=torch.int32, device=self.device)
             self.S = torch.empty(sz.S_bytes, dtype=torch.uint8, device=self.device) if sz.S_bytes else None
+            self.W = torch.empty(sz.workspace_bytes, dtype=torch.uint8, device=self.device) if sz.workspace_bytes else None
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             w = Weights((C.c_uint32 * 6)(*ct), (C.c_uint32 * 6)(*dir_mult), cost_one_log2, flags)
-            b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None, None)
+            b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None,
+                        self.W.data_ptr() if self.W is not None else None)
             h = C.c_void_p()
             rc = self._L.nhp_planner_create(C.byref(h), log2_n, log2_ntheta, float(R), C.byref(w), C.byref(b),
                                             C.c_void_p(self.stream.cuda_stream))

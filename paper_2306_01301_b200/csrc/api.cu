@@ -125,7 +125,7 @@ int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, nhp_sizes *out)
     out->V_bytes = nr * 4;
     out->C_bytes = nr / 8;
     out->S_bytes = (flags & NHP_FLAG_SOFT) ? nr : 0;
-    out->workspace_bytes = 0;
+    out->workspace_bytes = (flags & NHP_FLAG_SOFT) ? 3 * nr : 0;        // curve-major copies of S (S_left, S_right, S_line)
     return NHP_OK;
 }
 
@@ -137,13 +137,17 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     if (log2_n < 5 || log2_n > 12 || log2_ntheta < 5 || log2_ntheta > 12) return NHP_E_NOT_POW2;
     if (!(R_cells >= 1.0) || w->cost_one_log2 < 0 || w->cost_one_log2 > 16) return NHP_E_ARG;
     if ((double)(1 << log2_ntheta) < 2.0 * kPi * R_cells) return NHP_E_ANGRES;
-    if (!dev->V || !dev->C || ((w->flags & NHP_FLAG_SOFT) && !dev->S)) return NHP_E_BUFFER;
-    if (((uintptr_t)dev->V | (uintptr_t)dev->C | (uintptr_t)dev->S) & 255) return NHP_E_BUFFER;
+    if (!dev->V || !dev->C || ((w->flags & NHP_FLAG_SOFT) && (!dev->S || !dev->workspace))) return NHP_E_BUFFER;
+    if (((uintptr_t)dev->V | (uintptr_t)dev->C | (uintptr_t)dev->S | (uintptr_t)dev->workspace) & 255) return NHP_E_BUFFER;
     nhp_planner *p = new (std::nothrow) nhp_planner();
     if (!p) return NHP_E_ARG;
     p->log2_n = log2_n; p->log2_nt = log2_ntheta; p->n = 1 << log2_n; p->nt = 1 << log2_ntheta;
     p->R = R_cells; p->w = *w; p->stream = (cudaStream_t)cuda_stream;
     p->V = (uint32_t *)dev->V; p->C = (uint32_t *)dev->C; p->S = (w->flags & NHP_FLAG_SOFT) ? (uint8_t *)dev->S : nullptr;
+    if (p->S) {
+        const size_t nr = (size_t)p->n * p->n * p->nt;
+        p->S_left = (uint8_t *)dev->workspace; p->S_right = p->S_left + nr; p->S_line = p->S_right + nr;
+    }
     int rc = build_tables(p);
     if (rc == NHP_OK) rc = upload_tables(p);
     const size_t npx = (size_t)p->n * p->n;
@@ -151,7 +155,6 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     auto alloc = [&](void **ptr, size_t bytes) { if (rc == NHP_OK && cudaMalloc(ptr, bytes) != cudaSuccess) rc = NHP_E_CUDA; };
     alloc((void **)&p->d_hard, npx);
     alloc((void **)&p->d_soft, npx);
-    alloc((void **)&p->d_H, npx / 8);
     alloc((void **)&p->d_status, sizeof(int32_t) * 8);
     alloc((void **)&p->d_plan, sizeof(nhp_waypoint) * p->plan_cap);
     if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * 8) != cudaSuccess) rc = NHP_E_CUDA;
@@ -167,7 +170,8 @@ int nhp_planner_destroy(nhp_planner *p)
     if (!p) return NHP_E_ARG;
     cudaStreamSynchronize(p->stream);
     cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot);
-    cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_H);
+    cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
+    cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
     cudaFree(p->d_status); cudaFree(p->d_plan);
     if (p->h_status) cudaFreeHost(p->h_status);
     if (p->h_plan) cudaFreeHost(p->h_plan);
@@ -198,6 +202,8 @@ int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int m
     p->launches += launch_footprint_raster(p, mw, mh, ouq, ovq);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));            // mask_host may be freed by the caller after return
+    const int frc = finish_footprint(p);
+    if (frc != NHP_OK) return fail(p, frc, "building the footprint run tables failed");
     p->have_footprint = true;
     p->have_render = false;
     return NHP_OK;

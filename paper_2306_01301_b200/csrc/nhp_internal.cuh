@@ -20,6 +20,30 @@ constexpr uint32_t VI_BIG = VI_INF;            // added on edges that leave a bl
 
 enum { M_LF = 0, M_SF = 1, M_RB = 2, M_RF = 3, M_SB = 4, M_LB = 5 };
 
+#ifdef __CUDACC__
+// One vertex of a maneuver sweep, exactly the paper's line (Insert 5) in the internal encoding:
+//     v <- min(v, u + ct) + cx * B[i]              (arriving value v, stored value u, edge weight w at the SOURCE vertex)
+// with "infinity" leaving a blocked vertex (u == 0; blocked vertices are removed, DESIGN R10).
+// Three instructions, two of them on the min/max (DPX) pipe:
+//     e  = u + ct + w
+//     x  = min(v + w, e)                           unsigned: v <= 2^31 - 1 and w < 2^26, no wrap
+//     v' = max_signed(u + 0x7fffffff, x)           u == 0 -> INT_MAX ("infinite"); u >= 1 wraps negative -> x
+// Every value >= VI_INF is "infinite"; x < 2^31 because e < 2^31.
+__device__ __forceinline__ uint32_t nhp_chain_step(uint32_t v, uint32_t u, uint32_t w, uint32_t ct)
+{
+    const uint32_t e = u + ct + w;
+    const uint32_t x = __viaddmin_u32(v, w, e);
+    return (uint32_t)__viaddmax_s32((int)u, 0x7fffffff, (int)x);
+}
+
+// Soft edge weight (len_q * S) >> 4 (DESIGN R18) from len4 = len_q << 4 and byte `b` of a word of four S values:
+// one PRMT (S << 24) and one IMAD.HI.
+__device__ __forceinline__ uint32_t nhp_soft_weight(uint32_t len4, uint32_t packed, int b)
+{
+    return __umulhi(len4, __byte_perm(packed, 0u, (uint32_t)((b << 12) | 0x444)));
+}
+#endif
+
 struct DevTables {
     const int16_t *beta;    // [nt]      beta(Theta), eq (13)-(17) PAPER.md:233-262
     const int16_t *B;       // [nt][n]   B(y',Theta) = round(y' K(Theta))
@@ -34,6 +58,7 @@ struct nhp_planner {
     cudaStream_t stream = nullptr;
     uint32_t *V = nullptr, *C = nullptr;
     uint8_t *S = nullptr;
+    uint8_t *S_left = nullptr, *S_right = nullptr, *S_line = nullptr;   // curve-major copies of S (workspace), soft only
     // host tables (fp64 once, then integers)
     std::vector<int32_t> beta, B, cosq, sinq;
     std::vector<uint8_t> psi2, I;
@@ -51,7 +76,12 @@ struct nhp_planner {
     bool have_footprint = false;
     // images
     uint8_t *d_hard = nullptr, *d_soft = nullptr;
-    uint32_t *d_H = nullptr;       // [n][n/32] hard | wall, bit-packed rows
+    // run decomposition of E_Theta and the sparse tables of the image rows (render.cu)
+    int4 *d_runs = nullptr;        // (db, da_lo, second look-up offset, level) of every run, grouped by Theta
+    int32_t *d_run_off = nullptr;  // [nt + 1] first run of every Theta
+    int n_levels = 1, max_runs = 0;
+    uint32_t *d_Hk = nullptr;      // [levels][n][n/32] hard | wall, bit-packed rows; level k = OR over 2^k columns
+    uint8_t *d_Mk = nullptr;       // [levels][n][n]    soft image; level k = max over 2^k columns (soft only)
     bool have_render = false, have_run = false, canonical = false;
     int start[3] = {0, 0, 0};
     // plan extraction
@@ -94,9 +124,11 @@ struct ProfScope {
 
 // ---- kernel launchers (each returns the number of kernels it launched) ---------------------------
 int launch_footprint_raster(nhp_planner *p, int mw, int mh, int64_t ouq, int64_t ovq);
+int finish_footprint(nhp_planner *p);                 // host: run lists + table allocation; returns an NHP_ code
 int launch_render(nhp_planner *p, bool soft);
 int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);
 int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable
+int launch_soft_layouts(nhp_planner *p);              // softlayout.cu: S -> S_left, S_right, S_line

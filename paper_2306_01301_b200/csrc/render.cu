@@ -48,118 +48,204 @@ __global__ void pack_hard_kernel(uint32_t *__restrict__ H, const uint8_t *__rest
 }
 
 // ---------------------------------------------------------------------------------------------
-// Collision volume: C[Theta][j][i] = OR over (da, db) in E_Theta of H[(j+db)&M][(i+da)&M], 32 poses
-// per thread-word.  A block renders RJ rows of one Theta slice from a shared-memory copy of the
-// H rows it needs (RJ + 2 rad rows, wrapped).
+// Run decomposition of E_Theta (host, once per footprint): every row db of E_Theta is a union of runs
+// [da_lo, da_lo + len) of covered offsets (one run per row for a convex footprint, several for an
+// arbitrary mask).  OR / max over a run of any length is two look-ups in a sparse table of the image
+// rows: with k = floor(log2 len), T_k[a] = op(image[a .. a + 2^k - 1]) and
+//     op(image[x .. x + len - 1]) = op(T_k[x], T_k[x + len - 2^k])
+// (toroidal in a).  A pose then costs 2 look-ups per footprint ROW instead of one per footprint PIXEL.
 // ---------------------------------------------------------------------------------------------
-template <int RJ>
-__global__ void __launch_bounds__(256) render_collision_kernel(uint32_t *__restrict__ C, const uint32_t *__restrict__ H,
-                                                              const uint32_t *__restrict__ E, int n, int rad, int side,
-                                                              int sidew)
+int finish_footprint(nhp_planner *p)
 {
-    extern __shared__ uint32_t sm[];
-    const int nw = n >> 5, mx = n - 1, mw = nw - 1;
-    const int t = blockIdx.y, j0 = blockIdx.x * RJ;
-    const int rows = RJ + 2 * rad;
-    uint32_t *sE = sm;                       // [side][sidew]
-    uint32_t *sH = sm + side * sidew;        // [rows][nw]
-    for (int k = threadIdx.x; k < side * sidew; k += blockDim.x) sE[k] = E[(size_t)t * side * sidew + k];
-    for (int k = threadIdx.x; k < rows * nw; k += blockDim.x) {
-        const int r = k / nw, w = k - r * nw;
-        sH[k] = H[(size_t)((j0 - rad + r) & mx) * nw + w];
-    }
-    __syncthreads();
-    for (int k = threadIdx.x; k < RJ * nw; k += blockDim.x) {
-        const int jj = k / nw, iw = k - jj * nw;
-        uint32_t acc = 0;
+    const int nt = p->nt, side = p->side, sidew = p->sidew, rad = p->rad;
+    std::vector<uint32_t> E((size_t)nt * side * sidew);
+    if (cudaMemcpyAsync(E.data(), p->d_E, sizeof(uint32_t) * E.size(), cudaMemcpyDeviceToHost, p->stream) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return NHP_E_CUDA;
+    std::vector<int4> runs;
+    std::vector<int32_t> off(nt + 1, 0);
+    int maxk = 0, maxruns = 0;
+    for (int t = 0; t < nt; t++) {
+        off[t] = (int32_t)runs.size();
         for (int r = 0; r < side; r++) {
-            const uint32_t *hrow = sH + (jj + r) * nw;               // image row j + db, db = r - rad
-            for (int ew = 0; ew < sidew; ew++) {
-                uint32_t bits = sE[r * sidew + ew];
-                while (bits) {
-                    const int bpos = __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    const int x = iw * 32 + (ew * 32 + bpos - rad);  // first pixel column a = i + da
-                    const int w0 = (x >> 5) & mw;
-                    acc |= __funnelshift_r(hrow[w0], hrow[(w0 + 1) & mw], x & 31);
-                }
+            const uint32_t *row = &E[((size_t)t * side + r) * sidew];
+            int c = 0;
+            while (c < side) {
+                if (!((row[c >> 5] >> (c & 31)) & 1u)) { c++; continue; }
+                int e = c;
+                while (e < side && ((row[e >> 5] >> (e & 31)) & 1u)) e++;
+                const int len = e - c;
+                int k = 0;
+                while ((2 << k) <= len) k++;
+                runs.push_back(make_int4(r - rad, c - rad, len - (1 << k), k));      // db, da_lo, second look-up offset, level
+                maxk = k > maxk ? k : maxk;
+                c = e;
             }
         }
-        const int j = j0 + jj;
-        if (j == 0) acc = 0xffffffffu;
-        if (iw == 0) acc |= 1u;
-        C[((size_t)t * n + j) * nw + iw] = acc;
+        const int cnt = (int)runs.size() - off[t];
+        maxruns = cnt > maxruns ? cnt : maxruns;
     }
+    off[nt] = (int32_t)runs.size();
+    if (runs.empty()) runs.push_back(make_int4(0, 0, 0, 0));
+    cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
+    p->d_runs = nullptr; p->d_run_off = nullptr; p->d_Hk = nullptr; p->d_Mk = nullptr;
+    p->n_levels = maxk + 1;
+    p->max_runs = maxruns;
+    const size_t npx = (size_t)p->n * p->n;
+    if (cudaMalloc(&p->d_runs, sizeof(int4) * runs.size()) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaMalloc(&p->d_run_off, sizeof(int32_t) * (nt + 1)) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaMalloc(&p->d_Hk, (npx / 8) * p->n_levels) != cudaSuccess) return NHP_E_CUDA;
+    if (p->S && cudaMalloc(&p->d_Mk, npx * p->n_levels) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaMemcpyAsync(p->d_runs, runs.data(), sizeof(int4) * runs.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaMemcpyAsync(p->d_run_off, off.data(), sizeof(int32_t) * (nt + 1), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) return NHP_E_CUDA;
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) return NHP_E_CUDA;
+    return NHP_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Sparse tables of the image rows.  One block per image row b.
+//   hard: Hk[k][b][w], bit a of level k = OR of H[b][a .. a + 2^k - 1]      (level 0 = H, written by pack_hard_kernel)
+//   soft: Mk[k][b][a]        = max of soft[b][a .. a + 2^k - 1]
+// ---------------------------------------------------------------------------------------------
+__global__ void hard_levels_kernel(uint32_t *__restrict__ Hk, int n, int levels)
+{
+    extern __shared__ uint32_t sm[];                 // [2][nw]
+    const int nw = n >> 5, mw = nw - 1, b = blockIdx.x;
+    const size_t lvl = (size_t)n * nw;
+    uint32_t *cur = sm, *nxt = sm + nw;
+    for (int w = threadIdx.x; w < nw; w += blockDim.x) cur[w] = Hk[(size_t)b * nw + w];
+    __syncthreads();
+    for (int k = 1; k < levels; k++) {
+        const int s = 1 << (k - 1);
+        for (int w = threadIdx.x; w < nw; w += blockDim.x) {
+            uint32_t sh;
+            if (s < 32) sh = __funnelshift_r(cur[w], cur[(w + 1) & mw], s);
+            else sh = cur[(w + (s >> 5)) & mw];
+            const uint32_t v = cur[w] | sh;
+            nxt[w] = v;
+            Hk[k * lvl + (size_t)b * nw + w] = v;
+        }
+        __syncthreads();
+        uint32_t *t = cur; cur = nxt; nxt = t;
+    }
+}
+
+__global__ void soft_levels_kernel(uint32_t *__restrict__ Mk, const uint8_t *__restrict__ soft, int n, int levels)
+{
+    extern __shared__ uint32_t sm[];                 // [2][n/4]
+    const int nq = n >> 2, mq = nq - 1, b = blockIdx.x;
+    const size_t lvl = (size_t)n * nq;
+    uint32_t *cur = sm, *nxt = sm + nq;
+    const uint32_t *src = (const uint32_t *)(soft + (size_t)b * n);
+    for (int q = threadIdx.x; q < nq; q += blockDim.x) { cur[q] = src[q]; Mk[(size_t)b * nq + q] = src[q]; }
+    __syncthreads();
+    for (int k = 1; k < levels; k++) {
+        const int s = 1 << (k - 1);
+        for (int q = threadIdx.x; q < nq; q += blockDim.x) {
+            uint32_t sh;
+            if (s < 4) sh = __funnelshift_r(cur[q], cur[(q + 1) & mq], 8 * s);
+            else sh = cur[(q + (s >> 2)) & mq];
+            const uint32_t v = __vmaxu4(cur[q], sh);
+            nxt[q] = v;
+            Mk[k * lvl + (size_t)b * nq + q] = v;
+        }
+        __syncthreads();
+        uint32_t *t = cur; cur = nxt; nxt = t;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Collision volume: C[Theta][j][i] = OR over the runs of E_Theta of H[(j+db)&M][(i+da_lo .. )&M], 32 poses per
+// thread-word.  Block = 8 rows j x 32 words of one Theta slice (or the whole row if narrower).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t window32(const uint32_t *__restrict__ row, int x, int mw)
+{
+    const int w0 = (x >> 5) & mw;
+    return __funnelshift_r(__ldg(row + w0), __ldg(row + ((w0 + 1) & mw)), x & 31);
+}
+
+__global__ void __launch_bounds__(256) render_collision_kernel(uint32_t *__restrict__ C, const uint32_t *__restrict__ Hk,
+                                                              const int4 *__restrict__ runs, const int32_t *__restrict__ run_off, int n)
+{
+    extern __shared__ int4 srun[];
+    const int nw = n >> 5, mx = n - 1, mw = nw - 1;
+    const int t = blockIdx.z;
+    const int r0 = run_off[t], cnt = run_off[t + 1] - r0;
+    for (int k = threadIdx.x + threadIdx.y * blockDim.x; k < cnt; k += blockDim.x * blockDim.y) srun[k] = runs[r0 + k];
+    __syncthreads();
+    const int iw = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (iw >= nw) return;
+    const size_t lvl = (size_t)n * nw;
+    uint32_t acc = 0;
+    for (int k = 0; k < cnt; k++) {
+        const int4 r = srun[k];                                  // db, da_lo, second offset, level
+        const uint32_t *row = Hk + r.w * lvl + (size_t)((j + r.x) & mx) * nw;
+        const int x = (iw << 5) + r.y;
+        acc |= window32(row, x, mw) | window32(row, x + r.z, mw);
+    }
+    if (j == 0) acc = 0xffffffffu;                               // wall
+    if (iw == 0) acc |= 1u;
+    C[((size_t)t * n + j) * nw + iw] = acc;
 }
 
 // ---------------------------------------------------------------------------------------------
 // Soft volume: S = clamp(max over E_Theta of soft, 16, 255) (DESIGN R16), four poses per thread.
-// Tile of TX x TY poses with a halo of rad pixels staged in shared memory.
 // ---------------------------------------------------------------------------------------------
-constexpr int STX = 64, STY = 16;
-
-__global__ void __launch_bounds__(256) render_soft_kernel(uint8_t *__restrict__ S, const uint8_t *__restrict__ soft,
-                                                         const uint32_t *__restrict__ E, int n, int rad, int side,
-                                                         int sidew)
+__device__ __forceinline__ uint32_t window4(const uint32_t *__restrict__ row, int a, int mq)
 {
-    extern __shared__ uint32_t sm[];
-    const int mx = n - 1;
-    const int t = blockIdx.z, i0 = blockIdx.x * STX, j0 = blockIdx.y * STY;
-    const int pw = ((STX + 2 * rad + 6) >> 2) + 1;            // padded tile width in words
-    const int ph = STY + 2 * rad;
-    uint32_t *sE = sm;
-    uint8_t *sS = (uint8_t *)(sm + side * sidew);            // [ph][pw*4], column 0 <-> image column i0 - rad
-    for (int k = threadIdx.x; k < side * sidew; k += blockDim.x) sE[k] = E[(size_t)t * side * sidew + k];
-    for (int k = threadIdx.x; k < ph * pw * 4; k += blockDim.x) {
-        const int r = k / (pw * 4), c = k - r * (pw * 4);
-        sS[k] = soft[(size_t)((j0 - rad + r) & mx) * n + ((i0 - rad + c) & mx)];
-    }
+    const int q0 = (a >> 2) & mq;
+    return __funnelshift_r(__ldg(row + q0), __ldg(row + ((q0 + 1) & mq)), (a & 3) * 8);
+}
+
+__global__ void __launch_bounds__(256) render_soft_kernel(uint32_t *__restrict__ S4, const uint32_t *__restrict__ Mk,
+                                                         const int4 *__restrict__ runs, const int32_t *__restrict__ run_off, int n)
+{
+    extern __shared__ int4 srun[];
+    const int nq = n >> 2, mx = n - 1, mq = nq - 1;
+    const int t = blockIdx.z;
+    const int r0 = run_off[t], cnt = run_off[t + 1] - r0;
+    for (int k = threadIdx.x + threadIdx.y * blockDim.x; k < cnt; k += blockDim.x * blockDim.y) srun[k] = runs[r0 + k];
     __syncthreads();
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;  // 16 x 16 threads, 4 pixels each
-    uint32_t acc = 0x10101010u;                              // >= 16 = 1.0
-    const uint32_t *sw = (const uint32_t *)sS;
-    for (int r = 0; r < side; r++) {
-        const uint32_t *row = sw + (ty + r) * pw;
-        for (int ew = 0; ew < sidew; ew++) {
-            uint32_t bits = sE[r * sidew + ew];
-            while (bits) {
-                const int bpos = __ffs(bits) - 1;
-                bits &= bits - 1;
-                const int c = tx * 4 + ew * 32 + bpos;        // tile column of the first pixel: (i - i0) + da + rad
-                const uint32_t lo = row[c >> 2], hi = row[(c >> 2) + 1];
-                acc = __vmaxu4(acc, __funnelshift_r(lo, hi, (c & 3) * 8));
-            }
-        }
+    const int iq = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (iq >= nq) return;
+    const size_t lvl = (size_t)n * nq;
+    uint32_t acc = 0x10101010u;                                  // >= 16 = 1.0
+    for (int k = 0; k < cnt; k++) {
+        const int4 r = srun[k];
+        const uint32_t *row = Mk + r.w * lvl + (size_t)((j + r.x) & mx) * nq;
+        const int a = (iq << 2) + r.y;
+        acc = __vmaxu4(acc, __vmaxu4(window4(row, a, mq), window4(row, a + r.z, mq)));
     }
-    if (i0 + tx * 4 < n)                                     // n = 32: the 64-wide tile wraps onto itself
-        *(uint32_t *)(S + ((size_t)t * n + (j0 + ty)) * n + i0 + tx * 4) = acc;
+    S4[((size_t)t * n + j) * nq + iq] = acc;
 }
 
 int launch_render(nhp_planner *p, bool soft)
 {
-    const int n = p->n;
+    const int n = p->n, nw = n / 32, nq = n / 4;
+    int launches = 0;
     {
         ProfScope prof(p, 10);
-        pack_hard_kernel<<<dim3(n / 32, n), 32, 0, p->stream>>>(p->d_H, p->d_hard, n);
+        pack_hard_kernel<<<dim3(n / 32, n), 32, 0, p->stream>>>(p->d_Hk, p->d_hard, n);
+        hard_levels_kernel<<<n, nw < 32 ? 32 : nw, sizeof(uint32_t) * 2 * nw, p->stream>>>(p->d_Hk, n, p->n_levels);
+        launches += 2;
+        if (soft) {
+            soft_levels_kernel<<<n, nq < 256 ? nq : 256, sizeof(uint32_t) * 2 * nq, p->stream>>>((uint32_t *)p->d_Mk, p->d_soft, n, p->n_levels);
+            launches++;
+        }
     }
-    int launches = 1;
+    const size_t smem = sizeof(int4) * (size_t)(p->max_runs > 0 ? p->max_runs : 1);
     {
-        constexpr int RJ = 16;
         ProfScope prof(p, 6);
-        const size_t smem = sizeof(uint32_t) * ((size_t)p->side * p->sidew + (size_t)(RJ + 2 * p->rad) * (n / 32));
-        cudaFuncSetAttribute(render_collision_kernel<RJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        render_collision_kernel<RJ><<<dim3(n / RJ, p->nt), 256, smem, p->stream>>>(p->C, p->d_H, p->d_E, n, p->rad,
-                                                                                   p->side, p->sidew);
+        const dim3 block(nw < 32 ? nw : 32, 8);
+        render_collision_kernel<<<dim3(nw / block.x, n / 8, p->nt), block, smem, p->stream>>>(p->C, p->d_Hk, p->d_runs, p->d_run_off, n);
         launches++;
     }
     if (soft) {
-        const int pw = ((STX + 2 * p->rad + 6) >> 2) + 1, ph = STY + 2 * p->rad;
-        const size_t smem = sizeof(uint32_t) * ((size_t)p->side * p->sidew + (size_t)ph * pw);
-        cudaFuncSetAttribute(render_soft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         ProfScope prof(p, 7);
-        render_soft_kernel<<<dim3(n < STX ? 1 : n / STX, n / STY, p->nt), 256, smem, p->stream>>>(p->S, p->d_soft, p->d_E, n,
-                                                                                   p->rad, p->side, p->sidew);
+        const dim3 block(nq < 32 ? nq : 32, 8);
+        render_soft_kernel<<<dim3(nq / block.x, n / 8, p->nt), block, smem, p->stream>>>((uint32_t *)p->S, (const uint32_t *)p->d_Mk,
+                                                                                       p->d_runs, p->d_run_off, n);
         launches++;
+        launches += launch_soft_layouts(p);
     }
     return launches;
 }

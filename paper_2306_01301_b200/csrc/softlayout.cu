@@ -1,0 +1,77 @@
+// Curve-major copies of the soft volume S (second half).
+//
+// A sweep kernel walks along curves; its value volume V is staged tile by tile (sweep.cu, straight.cu), but the
+// soft multiplier S is one BYTE per vertex, too narrow to stage the same way (cp.async moves >= 4 bytes, and a warp
+// reading one byte per plane fetches a 32-byte sector for it).  So the renderer also writes S in the order the
+// sweeps consume it -- 32 consecutive steps of one curve are 32 consecutive bytes:
+//   S_left [y'][x'][Theta] = S[Theta][(y' + beta3(Theta)) & M][(x' + beta0(Theta)) & M]      left-turn curves, eq (18)
+//   S_right[y'][x'][Theta] = S[Theta][(y' + beta1(Theta)) & M][(x' + beta2(Theta)) & M]      right-turn curves, eq (18)
+//   S_line [Theta][x'][y'] = S at the vertex eq (23) gives for (x', y', Theta)                straight lines
+// Same bytes, same traffic per pose-update (1 B), three more volumes of N_R bytes in the caller's workspace.
+#include "nhp_internal.cuh"
+
+// One block = 32 neighbouring curves (x' = x0 .. x0 + 31 at one y') of one turn family: gather their N_theta planes
+// (32-byte row segments) into shared memory, write each curve's N_theta bytes out contiguously.
+__global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
+                                                              const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
+{
+    extern __shared__ __align__(16) uint8_t tile[];             // [32][nt + 16]
+    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2, stride = nt + 16;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int x0 = blockIdx.x << 5, yp = blockIdx.y;
+    for (int t = warp; t < nt; t += nwarps) {
+        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];
+        tile[lane * stride + t] = S[((((size_t)t << log2_n) + ((yp + bb) & mx)) << log2_n) + ((x0 + ba + lane) & mx)];
+    }
+    __syncthreads();
+    const int chunks = nt >> 4;                                 // 16-byte chunks per curve
+    uint8_t *out = Sout + (((size_t)yp << log2_n) + x0) * nt;
+    for (int c = threadIdx.x; c < 32 * chunks; c += blockDim.x) {
+        const int curve = c / chunks, q = c - curve * chunks;
+        *(uint4 *)(out + (size_t)curve * nt + 16 * q) = *(const uint4 *)(tile + curve * stride + 16 * q);
+    }
+}
+
+// One block = a 32 x 32 tile (x', y') of one Theta slice.
+__global__ void __launch_bounds__(256) soft_line_layout_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
+                                                              const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ, int log2_n)
+{
+    __shared__ uint8_t tile[32][33];
+    const int n = 1 << log2_n, mx = n - 1;
+    const int t = blockIdx.z, x0 = blockIdx.x << 5, y0 = blockIdx.y << 5;
+    const int lane = threadIdx.x, ty = threadIdx.y;
+    const int16_t *Bt = B + (size_t)t * n;
+    const uint8_t *St = S + ((size_t)t << (2 * log2_n));
+    uint8_t *Ot = Sout + ((size_t)t << (2 * log2_n));
+    if ((IJ[t] & 1) == 0) {
+        // eq (23), I = 0: (i, j) = (y', (x' + B(y')) & M): lane = y' is the memory-fast axis of both arrays
+        const int y = y0 + lane, b = Bt[y];
+        for (int r = ty; r < 32; r += 8) {
+            const int x = x0 + r;
+            Ot[((size_t)x << log2_n) + y] = St[((size_t)((x + b) & mx) << log2_n) + y];
+        }
+    } else {
+        // I = 1: (i, j) = ((x' + B(y')) & M, y'): read with lane = x', write with lane = y'
+        for (int r = ty; r < 32; r += 8) {
+            const int y = y0 + r;
+            tile[r][lane] = St[((size_t)y << log2_n) + ((x0 + lane + Bt[y]) & mx)];
+        }
+        __syncthreads();
+        for (int r = ty; r < 32; r += 8) Ot[((size_t)(x0 + r) << log2_n) + y0 + lane] = tile[lane][r];
+    }
+}
+
+int launch_soft_layouts(nhp_planner *p)
+{
+    const int n = p->n, nt = p->nt;
+    const size_t smem = (size_t)32 * (nt + 16);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(soft_turn_layout_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * (4096 + 16));
+        attr_set = true;
+    }
+    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
+    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
+    soft_line_layout_kernel<<<dim3(n / 32, n / 32, nt), dim3(32, 8), 0, p->stream>>>(p->S_line, p->S, p->d_B, p->d_IJ, p->log2_n);
+    return 3;
+}

@@ -136,32 +136,75 @@ __device__ __forceinline__ void tile_store(const uint32_t *tile, unsigned long l
     }
 }
 
-// Relax the 32 steps of a tile for this thread's line (Insert 5, PAPER.md:946-949, internal encoding):
-//   V[i] = min(v, u);  v = min(v, u + ct) + (blocked ? infinity : w)
-template <bool UP>
-__device__ __forceinline__ uint32_t tile_relax(uint32_t *line, uint32_t &v, uint32_t w, uint32_t ct)
+__device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
 {
-    uint32_t cm = 0;
-#pragma unroll
-    for (int s = 0; s < 32; s++) {
-        const int k = UP ? s : 31 - s;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_addr), "l"(gptr) : "memory");
+}
+
+// Relax the 32 steps of a tile for this thread's line (Insert 5, PAPER.md:946-949, internal encoding):
+//   V[i] = min(v, u);  v = min(v, u + ct) + (blocked ? infinity : w)          (nhp_chain_step)
+// Soft: w = (len_q * S) >> 4 per vertex, S from the line-major copy of the soft volume (sl: this line's 32 bytes).
+template <bool UP, bool SOFT, int S = 0>
+struct RelaxLoop {
+    static __device__ __forceinline__ void run(uint32_t *line, uint32_t &v, uint32_t w, uint32_t ct, const uint4 &s0, const uint4 &s1,
+                                               uint32_t &cm)
+    {
+        constexpr int k = UP ? S : 31 - S;
         const uint32_t u = line[k];
         if (v < u) { line[k] = v; cm |= 1u << k; }
-        v = __viaddmin_u32(u, ct, v) + (u != 0u ? w : VI_BIG);
+        uint32_t wk = w;
+        if (SOFT) {
+            const uint4 &q = (k < 16) ? s0 : s1;
+            const uint32_t word = ((k >> 2) & 3) == 0 ? q.x : ((k >> 2) & 3) == 1 ? q.y : ((k >> 2) & 3) == 2 ? q.z : q.w;
+            wk = nhp_soft_weight(w, word, k & 3);
+        }
+        v = nhp_chain_step(v, u, wk, ct);
+        RelaxLoop<UP, SOFT, S + 1>::run(line, v, w, ct, s0, s1, cm);
     }
+};
+template <bool UP, bool SOFT>
+struct RelaxLoop<UP, SOFT, 32> {
+    static __device__ __forceinline__ void run(uint32_t *, uint32_t &, uint32_t, uint32_t, const uint4 &, const uint4 &, uint32_t &) {}
+};
+
+template <bool UP, bool SOFT>
+__device__ __forceinline__ uint32_t tile_relax(uint32_t *line, const uint4 *sl, int lane, uint32_t &v, uint32_t w, uint32_t ct)
+{
+    uint32_t cm = 0;
+    uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
+    if (SOFT) { s0 = sl[lane]; s1 = sl[32 + lane]; }
+    RelaxLoop<UP, SOFT>::run(line, v, w, ct, s0, s1, cm);
     return cm;
 }
 
-template <bool XCLASS>
-__device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const int16_t *__restrict__ Bt, uint32_t *buf, int X0,
-                                           int lane, int log2_n, uint32_t w, uint32_t ct, bool pos, bool up)
+// One pipeline stage of a warp = the V tile and, with soft costs, the 32 x 32 bytes of S behind it ([half][lane] uint4).
+template <bool XCLASS, bool SOFT>
+__device__ __forceinline__ void stage_load(uint32_t stage, unsigned long long Vt, const uint8_t *__restrict__ Sl, const int16_t *__restrict__ Bt,
+                                           int T, int X0, int lane, int log2_n, bool pos)
 {
+    tile_load<XCLASS>(stage, Vt, Bt, T, X0, lane, log2_n, pos);
+    if (SOFT) {
+        // S_line[Theta][x'][y']: this lane's line, steps 32 T .. 32 T + 31 = 32 contiguous bytes.  In class-X tiles
+        // with K > 0 the rows are numbered downwards (tile_geometry), so thread `lane` owns line X0 + 31 - lane.
+        const int xl = (XCLASS && pos) ? 31 - lane : lane;
+        const uint8_t *g = Sl + (((size_t)(X0 + xl)) << log2_n) + 32 * T;
+        const uint32_t sa = stage + 4u * (uint32_t)ST_TILE_WORDS + 16u * (uint32_t)lane;
+        cp_async16(sa, g);
+        cp_async16(sa + 512u, g + 16);
+    }
+}
+
+template <bool XCLASS, bool SOFT>
+__device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const uint8_t *__restrict__ Sl, const int16_t *__restrict__ Bt,
+                                           uint32_t *buf, int X0, int lane, int log2_n, uint32_t w, uint32_t ct, bool pos, bool up)
+{
+    constexpr int SW = ST_TILE_WORDS + (SOFT ? 256 : 0);
     const int NT = 1 << (log2_n - 5);
     unsigned long long Vt = (unsigned long long)Vslice;
     asm volatile("" : "+l"(Vt));
     const uint32_t sbuf = (uint32_t)__cvta_generic_to_shared(buf);
     for (int s = 0; s < ST_NBUF - 1; s++) {
-        if (s < NT) tile_load<XCLASS>(sbuf + 4u * (uint32_t)(s * ST_TILE_WORDS), Vt, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos);
+        if (s < NT) stage_load<XCLASS, SOFT>(sbuf + 4u * (uint32_t)(s * SW), Vt, Sl, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos);
         cp_async_commit();
     }
     uint32_t v = VI_INF;
@@ -172,11 +215,13 @@ __device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const 
         __syncwarp();
         {   // prefetch tile s + NBUF - 1 into the buffer tile s - 1 has just left
             const int sn = s + ST_NBUF - 1;
-            if (sn < NT) tile_load<XCLASS>(sbuf + 4u * (uint32_t)(bn * ST_TILE_WORDS), Vt, Bt, up ? sn : NT - 1 - sn, X0, lane, log2_n, pos);
+            if (sn < NT) stage_load<XCLASS, SOFT>(sbuf + 4u * (uint32_t)(bn * SW), Vt, Sl, Bt, up ? sn : NT - 1 - sn, X0, lane, log2_n, pos);
             cp_async_commit();
         }
-        uint32_t *tile = buf + b * ST_TILE_WORDS;
-        const uint32_t cm = up ? tile_relax<true>(tile + lane * ST_STRIDE, v, w, ct) : tile_relax<false>(tile + lane * ST_STRIDE, v, w, ct);
+        uint32_t *tile = buf + b * SW;
+        const uint4 *sl = (const uint4 *)(tile + ST_TILE_WORDS);
+        const uint32_t cm = up ? tile_relax<true, SOFT>(tile + lane * ST_STRIDE, sl, lane, v, w, ct)
+                               : tile_relax<false, SOFT>(tile + lane * ST_STRIDE, sl, lane, v, w, ct);
         if (__any_sync(0xffffffffu, cm != 0u)) {
             __syncwarp();
             tile_store<XCLASS>(tile, Vt, Bt, up ? s : NT - 1 - s, X0, lane, log2_n, pos, cm);
@@ -186,11 +231,13 @@ __device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const 
     }
 }
 
-__global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict__ V, const int16_t *__restrict__ B,
-                                                            const uint8_t *__restrict__ IJ, const uint32_t *__restrict__ lenq,
-                                                            uint32_t ct, int log2_n, int is_forward)
+template <bool SOFT>
+__global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
+                                                            const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
+                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward)
 {
-    extern __shared__ uint32_t smem[];
+    extern __shared__ __align__(16) uint32_t smem[];
+    constexpr int SW = ST_TILE_WORDS + (SOFT ? 256 : 0);
     const int n = 1 << log2_n, t = blockIdx.y;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
@@ -199,10 +246,11 @@ __global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict
     const int16_t *Bt = B + (size_t)t * n;
     const bool pos = Bt[n - 1] >= 0;                                            // sign of K(Theta), eq (20)
     uint32_t *Vt = V + ((size_t)t << (2 * log2_n));
-    uint32_t *buf = smem + warp * (ST_NBUF * ST_TILE_WORDS);
-    const uint32_t w = lenq[t];
-    if (I == 0) band_sweep<true>(Vt, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
-    else band_sweep<false>(Vt, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
+    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) : nullptr;
+    uint32_t *buf = smem + warp * (ST_NBUF * SW);
+    const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
+    if (I == 0) band_sweep<true, SOFT>(Vt, Sl, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
+    else band_sweep<false, SOFT>(Vt, Sl, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
 }
 
 }  // namespace
@@ -211,17 +259,24 @@ __global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict
 int launch_straight_tile(nhp_planner *p, int m)
 {
     if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
-    if (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) return 0;               // soft variant: simple kernels for now
+    const bool soft = p->S != nullptr;
     const int n = p->n, nt = p->nt;
     const int bands = n / 32, warps = bands < 4 ? bands : 4;
-    const size_t smem = sizeof(uint32_t) * (size_t)warps * ST_NBUF * ST_TILE_WORDS;
+    const int sw = ST_TILE_WORDS + (soft ? 256 : 0);
+    const size_t smem = sizeof(uint32_t) * (size_t)warps * ST_NBUF * sw;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(straight_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * ST_NBUF * ST_TILE_WORDS * 4);
+        cudaFuncSetAttribute(straight_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * ST_NBUF * ST_TILE_WORDS * 4);
+        cudaFuncSetAttribute(straight_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * ST_NBUF * (ST_TILE_WORDS + 256) * 4);
         attr_set = true;
     }
     ProfScope prof(p, m);
-    straight_tile_kernel<<<dim3(bands / warps, nt), warps * 32, smem, p->stream>>>(p->V, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
-                                                                                   p->w.ct[m], p->log2_n, m == M_SF);
+    const dim3 grid(bands / warps, nt);
+    if (soft)
+        straight_tile_kernel<true><<<grid, warps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
+                                                                        p->w.ct[m], p->log2_n, m == M_SF);
+    else
+        straight_tile_kernel<false><<<grid, warps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
+                                                                         p->w.ct[m], p->log2_n, m == M_SF);
     return 1;
 }

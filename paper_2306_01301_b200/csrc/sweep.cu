@@ -183,73 +183,121 @@ static int launch_maneuver_simple(nhp_planner *p, int m)
 // ---------------------------------------------------------------------------------------------
 constexpr uint32_t D_CAP = 1u << 31;     // "a blocked vertex interrupts this section" as a summed edge cost
 
-// One vertex of a sweep with the arriving value v, exactly the paper's line (Insert 5):
-//     v = min(v, u + ct) + cx * B[i]
-// with the edge weight "infinite" at a blocked vertex (u == 0).  One DPX instruction + one add on the chain.
-__device__ __forceinline__ uint32_t chain_step(uint32_t v, uint32_t u, uint32_t w, uint32_t ct)
+// Edge weights of a section.  Hard obstacles only: one warp-uniform weight.  Soft: w = (len_q * S[p]) >> 4 per
+// vertex (DESIGN R18), S taken from the curve-major copy of the soft volume: 32 bytes per thread and section, read
+// 16 at a time in every pass (an L1 hit after the first) so that they do not occupy registers between passes.
+template <bool SOFT>
+struct SecW {
+    uint32_t len;          // hard: the edge weight itself; soft: len_q << 4
+    const uint4 *sp;       // soft: S of the section's 32 vertices, vertex k in byte k
+};
+
+__device__ __forceinline__ uint4 ld_s16(const uint4 *p)
 {
-    return __viaddmin_u32(u, ct, v) + (u != 0u ? w : VI_BIG);
+    uint4 q;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(q.x), "=r"(q.y), "=r"(q.z), "=r"(q.w) : "l"(p));
+    return q;
 }
 
-template <int L, bool UP>
-__device__ __forceinline__ uint32_t section_summary(const uint32_t (&col)[L], uint32_t w, uint32_t ct)
+template <bool SOFT, int K>
+__device__ __forceinline__ uint32_t sec_weight(const SecW<SOFT> &sw, const uint4 &q)
 {
-    uint32_t v = VI_INF;
-#pragma unroll
-    for (int s = 0; s < L; s++) v = chain_step(v, col[UP ? s : L - 1 - s], w, ct);
-    return v;
+    if (!SOFT) return sw.len;
+    const uint32_t word = ((K >> 2) & 3) == 0 ? q.x : ((K >> 2) & 3) == 1 ? q.y : ((K >> 2) & 3) == 2 ? q.z : q.w;
+    return nhp_soft_weight(sw.len, word, K & 3);
 }
 
-// Apply pass: the vertex keeps min(v, u); the value that travels on is the same chain step.
-template <int L, bool UP>
-__device__ __forceinline__ void section_apply(uint32_t (&col)[L], uint32_t w, uint32_t ct, uint32_t v, bool &changed)
-{
-#pragma unroll
-    for (int s = 0; s < L; s++) {
-        const int k = UP ? s : L - 1 - s;
-        const uint32_t u = col[k];
-        changed |= (v < u);                    // accumulates in a predicate: no register, no longer live range
-        col[k] = min(v, u);
-        v = chain_step(v, u, w, ct);
+template <int L, bool UP, bool SOFT, int S = 0>
+struct SecLoop {
+    static constexpr int k = UP ? S : L - 1 - S;
+    // summary pass: value leaving the section when it is entered with "infinity" (Sv of Insert 3)
+    // and, for soft weights, the summed edge cost across it (Sd)
+    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &v, uint32_t &d)
+    {
+        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
+        const uint32_t w = sec_weight<SOFT, k>(sw, q);
+        v = nhp_chain_step(v, col[k], w, ct);
+        if (SOFT) d += w;
+        SecLoop<L, UP, SOFT, S + 1>::summary(col, sw, q, ct, v, d);
     }
-}
+    // apply pass: the vertex keeps min(v, u); the value that travels on is the same chain step
+    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &v)
+    {
+        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
+        const uint32_t u = col[k];
+        col[k] = min(v, u);
+        v = nhp_chain_step(v, u, sec_weight<SOFT, k>(sw, q), ct);
+        SecLoop<L, UP, SOFT, S + 1>::apply(col, sw, q, ct, v);
+    }
+};
+template <int L, bool UP, bool SOFT>
+struct SecLoop<L, UP, SOFT, L> {
+    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &, uint32_t &) {}
+    static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &) {}
+};
 
 // carry into section `sec` of a closed curve cut into S (a power of two) sections, travel direction UP
 // (sec -> sec+1) or down: fold the other sections once around the curve, starting from section sec itself.
 template <bool UP>
-__device__ __forceinline__ uint32_t ripple_carry(const uint32_t *sM, const uint32_t *sD, int sec, int S, int lane)
+__device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int S, int lane)
 {
-    uint32_t c = sM[sec * 32 + lane];
-#pragma unroll 1
+    uint32_t c = sMD[sec * 32 + lane].x;
+#pragma unroll 4
     for (int r = 1; r < S; r++) {
-        const int q = (UP ? sec + r : sec - r) & (S - 1);
-        c = __viaddmin_u32(c, sD[q * 32 + lane], sM[q * 32 + lane]);
+        const uint2 md = sMD[((UP ? sec + r : sec - r) & (S - 1)) * 32 + lane];
+        c = __viaddmin_u32(c, md.y, md.x);
     }
     return c;
 }
 
-struct TurnPass { uint32_t w, ct; };
+// 64-bit checksum 3 * sum(col): the sums before and after the passes differ iff a vertex improved (values only
+// decrease).  mad.wide runs on the FMA pipe, which the sweeps leave idle; the min/max pipe is the busy one.
+template <int L>
+__device__ __forceinline__ unsigned long long tile_checksum(const uint32_t (&col)[L])
+{
+    unsigned long long acc = 0;
+#pragma unroll
+    for (int k = 0; k < L; k++) asm("mad.wide.u32 %0, %1, 3, %0;" : "+l"(acc) : "r"(col[k]));
+    return acc;
+}
 
-template <int L, int NPASS, bool UP0>
-__global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const int16_t *__restrict__ beta,
-                                                          int log2_n, int nt, int qa, int qb, TurnPass pa, TurnPass pb)
+struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4 (soft)
+
+template <int L, bool UP, bool SOFT>
+__device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool interrupted, uint2 *sMD,
+                                              int sec, int S, int lane)
+{
+    sw.len = pass.w;
+    uint32_t m = VI_INF, d = 0;
+    SecLoop<L, UP, SOFT>::summary(col, sw, make_uint4(0, 0, 0, 0), pass.ct, m, d);
+    if (!SOFT) d = (uint32_t)L * pass.w;
+    sMD[sec * 32 + lane] = make_uint2(m, interrupted ? D_CAP : d);
+    __syncthreads();
+    uint32_t v = ripple_carry<UP>(sMD, sec, S, lane);
+    // opaque copy of the weight: otherwise the per-vertex values of the summary pass are kept alive for the apply pass
+    asm volatile("" : "+r"(sw.len));
+    SecLoop<L, UP, SOFT>::apply(col, sw, make_uint4(0, 0, 0, 0), pass.ct, v);
+}
+
+template <int L, int NPASS, bool UP0, bool SOFT>
+__global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Scurve,
+                                                          const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb,
+                                                          TurnPass pa, TurnPass pb)
 {
     extern __shared__ uint32_t smem[];
     const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
     uint2 *soff = (uint2 *)smem;                              // [nt] (row base index, first column) of the tile
-    uint32_t *sM = smem + 2 * nt, *sD = sM + 2 * S * 32;      // [2][S][32] each
+    uint2 *sMD = soff + nt;                                   // [2][S][32] (M, D) of every section, one set per maneuver
     const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
     for (int t = threadIdx.x; t < nt; t += blockDim.x) {
         const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
         soff[t] = make_uint2((uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n)), (uint32_t)((x0 + ba) & mx));
     }
+    SecW<SOFT> sw;
+    sw.len = 0;
+    sw.sp = SOFT ? (const uint4 *)(Scurve + ((((size_t)yp << log2_n) + x0 + lane) * nt + sec * L)) : nullptr;
     __syncthreads();
-    // The apply passes take their weight through an opaque copy: otherwise the compiler keeps the 32 per-vertex
-    // edge weights of the summary pass alive for the apply pass (common sub-expression) and spills them.
-    const uint32_t wa = pa.w, ctwa = pa.ct, wb = pb.w, ctwb = pb.ct;
-    uint32_t wa2 = pa.w, wb2 = pb.w;
-    asm volatile("" : "+r"(wa2), "+r"(wb2));
     uint32_t col[L];
 #pragma unroll
     for (int k = 0; k < L; k++) {
@@ -261,19 +309,10 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
 #pragma unroll
     for (int k = 1; k < L; k++) lowest = min(lowest, col[k]);
     const bool interrupted = (lowest == 0u);
-    bool changed = false;
-    sM[sec * 32 + lane] = section_summary<L, UP0>(col, wa, ctwa);
-    sD[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wa;
-    __syncthreads();
-    section_apply<L, UP0>(col, wa2, ctwa, ripple_carry<UP0>(sM, sD, sec, S, lane), changed);
-    if (NPASS == 2) {
-        uint32_t *sM2 = sM + S * 32, *sD2 = sD + S * 32;
-        sM2[sec * 32 + lane] = section_summary<L, !UP0>(col, wb, ctwb);
-        sD2[sec * 32 + lane] = interrupted ? D_CAP : (uint32_t)L * wb;
-        __syncthreads();
-        section_apply<L, !UP0>(col, wb2, ctwb, ripple_carry<!UP0>(sM2, sD2, sec, S, lane), changed);
-    }
-    if (changed) {
+    const unsigned long long before = tile_checksum<L>(col);
+    turn_maneuver<L, UP0, SOFT>(col, sw, pa, interrupted, sMD, sec, S, lane);
+    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT>(col, sw, pb, interrupted, sMD + S * 32, sec, S, lane);
+    if (tile_checksum<L>(col) != before) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // recompute the addresses: keeping 64 of them alive across the passes spills
 #pragma unroll
@@ -288,7 +327,6 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
 static int turn_tile_L(const nhp_planner *p)
 {
     if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
-    if (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) return 0;            // soft variant: simple kernels for now
     if ((size_t)p->n * p->n * p->nt > ((size_t)1 << 32)) return 0;
     return p->nt <= 1024 ? 32 : 0;
 }
@@ -297,21 +335,26 @@ static int turn_tile_L(const nhp_planner *p)
 static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
 {
     const int n = p->n, nt = p->nt, S = nt / L;
+    const bool soft = p->S != nullptr;
     const bool left = (ma == M_LF || ma == M_LB);
     const int qa = left ? 0 : 2, qb = left ? 3 : 1;
     const bool up = (ma == M_LF || ma == M_RB);
     auto pass = [&](int m) {
         TurnPass t{0, 0};
-        if (m >= 0) { t.w = p->len_q[(size_t)m * nt]; t.ct = p->w.ct[m]; }       // turn edge length does not depend on Theta (l.334)
+        // turn edge length does not depend on Theta (l.334); soft kernels take len_q << 4 (nhp_soft_weight)
+        if (m >= 0) { t.w = soft ? p->len_q[(size_t)m * nt] << 4 : p->len_q[(size_t)m * nt]; t.ct = p->w.ct[m]; }
         return t;
     };
     const TurnPass pa = pass(ma), pb = pass(mb);
+    const uint8_t *Sc = left ? p->S_left : p->S_right;
     const dim3 grid(n / 32, n), block(32 * S);
-    const size_t smem = sizeof(uint32_t) * (2 * (size_t)nt + 4 * (size_t)S * 32);
+    const size_t smem = sizeof(uint2) * ((size_t)nt + 2 * (size_t)S * 32);
     ProfScope prof(p, mb >= 0 ? 11 : ma);
-#define NHP_TT(LL, NP, UP) turn_tile_kernel<LL, NP, UP><<<grid, block, smem, p->stream>>>(p->V, p->d_beta, p->log2_n, nt, qa, qb, pa, pb)
-    if (mb >= 0) { if (up) NHP_TT(32, 2, true); else NHP_TT(32, 2, false); }
-    else { if (up) NHP_TT(32, 1, true); else NHP_TT(32, 1, false); }
+#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb)
+#define NHP_TT2(NP, UP) do { if (soft) NHP_TT(NP, UP, true); else NHP_TT(NP, UP, false); } while (0)
+    if (mb >= 0) { if (up) NHP_TT2(2, true); else NHP_TT2(2, false); }
+    else { if (up) NHP_TT2(1, true); else NHP_TT2(1, false); }
+#undef NHP_TT2
 #undef NHP_TT
     return 1;
 }
