@@ -50,6 +50,21 @@ def workload_name(sc, n_cycles):
             f"N_T={n_cycles}, {'soft+hard' if sc.soft is not None else 'hard'} obstacles")
 
 
+def measured_traffic(config, slot):
+    """dram bytes per launch of `slot` from the committed ncu capture (profiles/traffic.csv), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for ln in f:
+                if ln.startswith("#") or not ln.strip():
+                    continue
+                c, k, b, src = ln.strip().split(",")
+                if int(c) == config and k == slot:
+                    return {"bytes_per_launch": int(b), "source": src}
+    except OSError:
+        pass
+    return None
+
+
 def peak_hbm():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     try:
@@ -192,6 +207,7 @@ def run_ours(args):
     achieved = per_launch_bytes / (dom_ms / max(dom_n, 1) * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
+    traffic = measured_traffic(args.config, dom)
     out = {
         "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
@@ -207,7 +223,8 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(16 * 4096 + 32)},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": n_r * (2 if dom == "turn_pair" else 1), "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "frac": achieved / peak, "traffic": traffic["bytes_per_launch"] if traffic else None,
+                     "traffic_source": traffic["source"] if traffic else None, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
                      "launches_timed": int(dom_n),
                      "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
