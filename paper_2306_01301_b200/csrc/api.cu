@@ -97,6 +97,12 @@ int upload_tables(nhp_planner *p)
         rot[4 * t + 2] = p->psi2[t]; rot[4 * t + 3] = p->psi2[(t + nt / 4) & (nt - 1)];   // 2 Psi0, 2 Psi1, eq (16)
     }
     for (size_t k = 0; k < B16.size(); k++) B16[k] = (int16_t)p->B[k];
+    std::vector<int16_t> tlist;
+    for (int t = 0; t < nt; t++) if (p->I[t] == 0) tlist.push_back((int16_t)t);
+    p->n_xslices = (int)tlist.size();
+    for (int t = 0; t < nt; t++) if (p->I[t] != 0) tlist.push_back((int16_t)t);
+    CU(cudaMalloc(&p->d_tlist, sizeof(int16_t) * nt));
+    CU(cudaMemcpyAsync(p->d_tlist, tlist.data(), sizeof(int16_t) * nt, cudaMemcpyHostToDevice, p->stream));
     CU(cudaMalloc(&p->d_beta, sizeof(int16_t) * nt));
     CU(cudaMalloc(&p->d_B, sizeof(int16_t) * B16.size()));
     CU(cudaMalloc(&p->d_lenq, sizeof(uint32_t) * 6 * nt));
@@ -169,7 +175,7 @@ int nhp_planner_destroy(nhp_planner *p)
 {
     if (!p) return NHP_E_ARG;
     cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot);
+    cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
     cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
     cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
     cudaFree(p->d_status); cudaFree(p->d_plan);

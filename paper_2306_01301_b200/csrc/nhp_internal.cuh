@@ -68,6 +68,8 @@ struct nhp_planner {
     int16_t *d_beta = nullptr, *d_B = nullptr;
     uint32_t *d_lenq = nullptr;
     uint8_t *d_IJ = nullptr;
+    int16_t *d_tlist = nullptr;    // [nt] slices with I = 0 first (n_xslices of them), then those with I = 1
+    int n_xslices = 0;
     int32_t *d_rot = nullptr;      // [nt][4] cosq, sinq, 2*Psi0, 2*Psi1
     // footprint
     int rad = 0, side = 0, sidew = 0;

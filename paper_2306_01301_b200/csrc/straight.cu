@@ -141,6 +141,13 @@ __device__ __forceinline__ void cp_async16(uint32_t smem_addr, const void *gptr)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(smem_addr), "l"(gptr) : "memory");
 }
 
+__device__ __forceinline__ uint4 ld_nc16(const uint8_t *p)
+{
+    uint4 q;
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(q.x), "=r"(q.y), "=r"(q.z), "=r"(q.w) : "l"(p));
+    return q;
+}
+
 // Relax the 32 steps of a tile for this thread's line (Insert 5, internal encoding):
 //   V[i] = min(v, u);  v = min(v, u + ct) + (blocked ? infinity : w)          (nhp_chain_step)
 // Soft: w = (len_q * S) >> 4 per vertex, S from the line-major copy of the soft volume (sl: this line's 32 bytes).
@@ -234,11 +241,12 @@ __device__ __forceinline__ void band_sweep(uint32_t *__restrict__ Vslice, const 
 template <bool SOFT>
 __global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
                                                             const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
+                                                            const int16_t *__restrict__ tlist,
                                                             const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     constexpr int SW = ST_TILE_WORDS + (SOFT ? 256 : 0);
-    const int n = 1 << log2_n, t = blockIdx.y;
+    const int n = 1 << log2_n, t = tlist[blockIdx.y];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
     const int I = IJ[t] & 1, jpos = (IJ[t] >> 1) & 1;
@@ -253,9 +261,66 @@ __global__ void __launch_bounds__(128) straight_tile_kernel(uint32_t *__restrict
     else band_sweep<false, SOFT>(Vt, Sl, Bt, buf, X0, lane, log2_n, w, ct, pos, up);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Slices with I = 1 (eq (19)): the sweep step is the ROW j and line x' sits at column
+// (x' + B(j)) & mask, so a warp that owns 32 neighbouring lines reads, at every step, one (misaligned, possibly
+// wrapping) 128-byte row segment in which lane l's word already IS line l's vertex: no transposition, no shared
+// memory.  A tile of 32 steps lives in 32 registers per thread (plain LDG: 1.8 cycles per warp instruction against
+// the 8 of a 4-byte cp.async, profiles/r01_tile_kernels.md); all warps of the launch are resident at once and the
+// loads of one warp's tile overlap the chains of the others.  Vertices that improve are stored from the thread
+// that owns them.
+// ---------------------------------------------------------------------------------------------
+template <bool SOFT>
+__global__ void __launch_bounds__(128, 8) straight_rows_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
+                                                            const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
+                                                            const int16_t *__restrict__ tlist,
+                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward)
+{
+    const int n = 1 << log2_n, mx = n - 1, t = tlist[blockIdx.y];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
+    const int jpos = (IJ[t] >> 1) & 1;
+    const bool up = (is_forward == jpos);                                       // eq (24)
+    const int16_t *Bt = B + (size_t)t * n;
+    unsigned long long Vt = (unsigned long long)(V + ((size_t)t << (2 * log2_n)));
+    asm volatile("" : "+l"(Vt));
+    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) + ((size_t)(X0 + lane) << log2_n) : nullptr;
+    const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
+    const uint32_t c0 = (uint32_t)(X0 + lane);
+    const int NT = n >> 5;
+    uint32_t v = VI_INF;
+#pragma unroll 1
+    for (int s = 0; s < NT; s++) {
+        const int T = up ? s : NT - 1 - s;
+        const int bmine = Bt[32 * T + lane];
+        const uint32_t row0 = (uint32_t)(32 * T) << log2_n;
+        uint32_t u[32];
+#pragma unroll
+        for (int k = 0; k < 32; k++) {
+            const int b = __shfl_sync(0xffffffffu, bmine, k);
+            const uint32_t off = row0 + ((uint32_t)k << log2_n) + ((c0 + (uint32_t)b) & (uint32_t)mx);
+            u[k] = *(const uint32_t *)(Vt + 4ull * off);
+        }
+        uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
+        if (SOFT) { s0 = ld_nc16(Sl + 32 * T); s1 = ld_nc16(Sl + 32 * T + 16); }
+        uint32_t cm = 0;
+        if (up) RelaxLoop<true, SOFT>::run(u, v, w, ct, s0, s1, cm);
+        else RelaxLoop<false, SOFT>::run(u, v, w, ct, s0, s1, cm);
+        if (__any_sync(0xffffffffu, cm != 0u)) {
+#pragma unroll
+            for (int k = 0; k < 32; k++) {
+                const int b = __shfl_sync(0xffffffffu, bmine, k);
+                const uint32_t off = row0 + ((uint32_t)k << log2_n) + ((c0 + (uint32_t)b) & (uint32_t)mx);
+                if ((cm >> k) & 1u) st_global(Vt, off, u[k]);
+            }
+        }
+    }
+}
+
 }  // namespace
 
-// SF or SB over the whole volume; returns the number of kernels launched (0 = not applicable, use the simple kernel)
+// SF or SB over the whole volume: one launch for the slices with I = 0 (tiles transposed through shared memory)
+// and one for those with I = 1 (tiles in registers).  Returns the number of kernels launched (0 = not applicable).
 int launch_straight_tile(nhp_planner *p, int m)
 {
     if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
@@ -271,12 +336,16 @@ int launch_straight_tile(nhp_planner *p, int m)
         attr_set = true;
     }
     ProfScope prof(p, m);
-    const dim3 grid(bands / warps, nt);
-    if (soft)
-        straight_tile_kernel<true><<<grid, warps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
-                                                                        p->w.ct[m], p->log2_n, m == M_SF);
-    else
-        straight_tile_kernel<false><<<grid, warps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_lenq + (size_t)m * nt,
-                                                                         p->w.ct[m], p->log2_n, m == M_SF);
-    return 1;
+    const uint32_t *lenq = p->d_lenq + (size_t)m * nt;
+    const int nx = p->n_xslices, ny = nt - nx;
+    const dim3 gx(bands / warps, nx), gy(bands / warps, ny);
+    const int fwd = (m == M_SF);
+    if (soft) {
+        straight_tile_kernel<true><<<gx, warps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd);
+        straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd);
+    } else {
+        straight_tile_kernel<false><<<gx, warps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd);
+        straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd);
+    }
+    return 2;
 }
