@@ -36,6 +36,27 @@ __device__ __forceinline__ uint32_t nhp_chain_step(uint32_t v, uint32_t u, uint3
     return (uint32_t)__viaddmax_s32((int)u, 0x7fffffff, (int)x);
 }
 
+// The same line with the arriving value carried as a = v - ct ("transition cost not charged yet") and the edge weight
+// of the PREVIOUS vertex still pending: t = min(a, u) is the value at the vertex before its own edge, so
+//     t_k   = min(t_{k-1} + w_{k-1}, u_k)                           one DPX op, no separate addition
+//     out_k = min(v_k, u_k) = min(t_k + ct, u_k)                    one DPX op (u_k <= u_k + ct)
+//     t_k  <- "infinite" if the vertex is blocked (u_k == 0)        one DPX op (signed max against u + INT_MAX)
+// a never goes negative: every finite v is some u_j + ct + (edge weights) >= 1 + ct.  No wrap: t <= 2^31 - 1,
+// w, ct < 2^26.  Identical integers to nhp_chain_step (a + ct = v), two / three ALU ops per vertex instead of
+// three / four.
+__device__ __forceinline__ uint32_t nhp_arrive(uint32_t t_prev, uint32_t w_prev, uint32_t u)
+{
+    return __viaddmin_u32(t_prev, w_prev, u);
+}
+__device__ __forceinline__ uint32_t nhp_keep(uint32_t t, uint32_t ct, uint32_t u)
+{
+    return __viaddmin_u32(t, ct, u);
+}
+__device__ __forceinline__ uint32_t nhp_gate(uint32_t t, uint32_t u)
+{
+    return (uint32_t)__viaddmax_s32((int)u, 0x7fffffff, (int)t);
+}
+
 // Soft edge weight (len_q * S) >> 4 (DESIGN R18) from len4 = len_q << 4 and byte `b` of a word of four S values:
 // one PRMT (S << 24) and one IMAD.HI.
 __device__ __forceinline__ uint32_t nhp_soft_weight(uint32_t len4, uint32_t packed, int b)

@@ -210,34 +210,39 @@ __device__ __forceinline__ uint32_t sec_weight(const SecW<SOFT> &sw, const uint4
 template <int L, bool UP, bool SOFT, int S = 0>
 struct SecLoop {
     static constexpr int k = UP ? S : L - 1 - S;
-    // summary pass: value leaving the section when it is entered with "infinity" (Sv of Insert 3)
-    // and, for soft weights, the summed edge cost across it (Sd)
-    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &v, uint32_t &d)
-    {
-        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
-        const uint32_t w = sec_weight<SOFT, k>(sw, q);
-        v = nhp_chain_step(v, col[k], w, ct);
-        if (SOFT) d += w;
-        SecLoop<L, UP, SOFT, S + 1>::summary(col, sw, q, ct, v, d);
-    }
-    // apply pass: the vertex keeps min(v, u); the value that travels on is the same chain step
-    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &v)
+    // summary pass: the section entered with "infinity" (Sv of Insert 3); t is the value AT the
+    // vertex before its own edge (nhp_arrive / nhp_gate), wp the pending weight of the vertex behind it; for soft
+    // weights d sums the edge costs across the section (Sd)
+    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t &t, uint32_t &wp, uint32_t &d)
     {
         if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
         const uint32_t u = col[k];
-        col[k] = min(v, u);
-        v = nhp_chain_step(v, u, sec_weight<SOFT, k>(sw, q), ct);
-        SecLoop<L, UP, SOFT, S + 1>::apply(col, sw, q, ct, v);
+        t = nhp_gate(nhp_arrive(t, wp, u), u);
+        wp = sec_weight<SOFT, k>(sw, q);
+        if (SOFT) d += wp;
+        SecLoop<L, UP, SOFT, S + 1>::summary(col, sw, q, t, wp, d);
+    }
+    // apply pass: the vertex keeps min(v, u), then the same step
+    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &t, uint32_t &wp)
+    {
+        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
+        const uint32_t u = col[k];
+        t = nhp_arrive(t, (!SOFT && S == 0) ? 0u : wp, u);
+        col[k] = nhp_keep(t, ct, u);
+        t = nhp_gate(t, u);
+        if (SOFT) wp = sec_weight<SOFT, k>(sw, q);
+        SecLoop<L, UP, SOFT, S + 1>::apply(col, sw, q, ct, t, wp);
     }
 };
 template <int L, bool UP, bool SOFT>
 struct SecLoop<L, UP, SOFT, L> {
-    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &, uint32_t &) {}
-    static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &) {}
+    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t &, uint32_t &, uint32_t &) {}
+    static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &, uint32_t &) {}
 };
 
 // carry into section `sec` of a closed curve cut into S (a power of two) sections, travel direction UP
 // (sec -> sec+1) or down: fold the other sections once around the curve, starting from section sec itself.
+// M <= 2^31 - 1 and D <= 2^31, so c + D never wraps.
 template <bool UP>
 __device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int S, int lane)
 {
@@ -250,76 +255,120 @@ __device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int 
     return c;
 }
 
-// 64-bit checksum 3 * sum(col): the sums before and after the passes differ iff a vertex improved (values only
-// decrease).  mad.wide runs on the FMA pipe, which the sweeps leave idle; the min/max pipe is the busy one.
+// 64-bit checksum sum(col): the sums before and after the passes differ iff a vertex improved (values only
+// decrease).  mad.wide runs on the FMA pipe, which the sweeps leave idle; the min/max pipe is the busy one.  The
+// multiplier 1 comes from the kernel parameters: ptxas turns a multiplication by a KNOWN 1 into ALU-pipe
+// IADD3 / IADD3.X pairs.
 template <int L>
-__device__ __forceinline__ unsigned long long tile_checksum(const uint32_t (&col)[L])
+__device__ __forceinline__ unsigned long long tile_checksum(const uint32_t (&col)[L], uint32_t one)
 {
     unsigned long long acc = 0;
 #pragma unroll
-    for (int k = 0; k < L; k++) asm("mad.wide.u32 %0, %1, 3, %0;" : "+l"(acc) : "r"(col[k]));
+    for (int k = 0; k < L; k++) asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(col[k]), "r"(one));
     return acc;
 }
 
 struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4 (soft)
 
+// One maneuver over the tile.  All values travel as a = v - ct (nhp_arrive): the section summary M is the value
+// arriving at the first vertex of the NEXT section, D the summed edge cost across the section.
 template <int L, bool UP, bool SOFT>
 __device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool interrupted, uint2 *sMD,
                                               int sec, int S, int lane)
 {
     sw.len = pass.w;
-    uint32_t m = VI_INF, d = 0;
-    SecLoop<L, UP, SOFT>::summary(col, sw, make_uint4(0, 0, 0, 0), pass.ct, m, d);
+    uint32_t t = VI_INF, wp = SOFT ? 0u : pass.w, d = 0;
+    SecLoop<L, UP, SOFT>::summary(col, sw, make_uint4(0, 0, 0, 0), t, wp, d);
     if (!SOFT) d = (uint32_t)L * pass.w;
-    sMD[sec * 32 + lane] = make_uint2(m, interrupted ? D_CAP : d);
+    sMD[sec * 32 + lane] = make_uint2(__viaddmin_u32(t, wp, 0x7fffffffu), interrupted ? D_CAP : d);
     __syncthreads();
-    uint32_t v = ripple_carry<UP>(sMD, sec, S, lane);
+    t = ripple_carry<UP>(sMD, sec, S, lane);
     // opaque copy of the weight: otherwise the per-vertex values of the summary pass are kept alive for the apply pass
     asm volatile("" : "+r"(sw.len));
-    SecLoop<L, UP, SOFT>::apply(col, sw, make_uint4(0, 0, 0, 0), pass.ct, v);
+    wp = SOFT ? 0u : sw.len;
+    SecLoop<L, UP, SOFT>::apply(col, sw, make_uint4(0, 0, 0, 0), pass.ct, t, wp);
+}
+
+// Row addressing of a tile: so[t] = element index of the tile's first vertex in plane t (row base + first column).
+// A tile whose 32 columns never cross the seam i = N-1 -> 0 ("!wraps", CTA-uniform) addresses vertex (t, lane) as
+// (V + lane)[so[t]]: one IMAD.WIDE per vertex; otherwise the column is wrapped per lane (one add + one bit-select more).
+template <int L, bool WRAPS>
+__device__ __forceinline__ void tile_rows_load(uint32_t (&col)[L], const uint32_t *__restrict__ V, const uint32_t *so, int lane, uint32_t mx)
+{
+    unsigned long long Vl = (unsigned long long)(V + (WRAPS ? 0 : lane));
+    asm volatile("" : "+l"(Vl));            // opaque per-thread base: address = one IMAD.WIDE (base + 4 * index)
+    const uint4 *so4 = (const uint4 *)so;
+#pragma unroll
+    for (int q = 0; q < L / 4; q++) {
+        const uint4 o = so4[q];
+        const uint32_t oo[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+        for (int e = 0; e < 4; e++) {
+            uint32_t idx = oo[e];
+            if (WRAPS) idx = ((idx + (uint32_t)lane) & mx) | (idx & ~mx);
+            asm volatile("ld.global.u32 %0, [%1];" : "=r"(col[4 * q + e]) : "l"(Vl + 4ull * idx));
+        }
+    }
+}
+
+template <int L, bool WRAPS>
+__device__ __forceinline__ void tile_rows_store(const uint32_t (&col)[L], uint32_t *__restrict__ V, const uint32_t *so, int lane, uint32_t mx)
+{
+    unsigned long long Vl = (unsigned long long)(V + (WRAPS ? 0 : lane));
+    asm volatile("" : "+l"(Vl));
+    const uint4 *so4 = (const uint4 *)so;
+#pragma unroll
+    for (int q = 0; q < L / 4; q++) {
+        const uint4 o = so4[q];
+        const uint32_t oo[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+        for (int e = 0; e < 4; e++) {
+            uint32_t idx = oo[e];
+            if (WRAPS) idx = ((idx + (uint32_t)lane) & mx) | (idx & ~mx);
+            asm volatile("st.global.u32 [%0], %1;" ::"l"(Vl + 4ull * idx), "r"(col[4 * q + e]) : "memory");
+        }
+    }
 }
 
 template <int L, int NPASS, bool UP0, bool SOFT>
 __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Scurve,
                                                           const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb,
-                                                          TurnPass pa, TurnPass pb)
+                                                          TurnPass pa, TurnPass pb, uint32_t one)
 {
-    extern __shared__ uint32_t smem[];
+    extern __shared__ __align__(16) uint32_t smem[];
     const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
-    uint2 *soff = (uint2 *)smem;                              // [nt] (row base index, first column) of the tile
-    uint2 *sMD = soff + nt;                                   // [2][S][32] (M, D) of every section, one set per maneuver
+    uint32_t *so = smem;                                      // [nt] element index of the tile's first vertex in every plane
+    uint2 *sMD = (uint2 *)(so + nt);                          // [2][S][32] (M, D) of every section, one set per maneuver
     const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
+    int seam = 0;
     for (int t = threadIdx.x; t < nt; t += blockDim.x) {
         const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
-        soff[t] = make_uint2((uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n)), (uint32_t)((x0 + ba) & mx));
+        const int c0 = (x0 + ba) & mx;
+        so[t] = (uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n) + c0);
+        seam |= (c0 > mx - 31);
     }
     SecW<SOFT> sw;
     sw.len = 0;
     sw.sp = SOFT ? (const uint4 *)(Scurve + ((((size_t)yp << log2_n) + x0 + lane) * nt + sec * L)) : nullptr;
-    __syncthreads();
+    const bool wraps = __syncthreads_or(seam) != 0;
     uint32_t col[L];
-#pragma unroll
-    for (int k = 0; k < L; k++) {
-        const uint2 o = soff[sec * L + k];
-        col[k] = V[o.x + ((o.y + lane) & mx)];
-    }
+    if (!wraps) tile_rows_load<L, false>(col, V, so + sec * L, lane, (uint32_t)mx);
+    else tile_rows_load<L, true>(col, V, so + sec * L, lane, (uint32_t)mx);
     // blocked vertices never change, so "does a blocked vertex interrupt my section" is decided once
     uint32_t lowest = col[0];
 #pragma unroll
-    for (int k = 1; k < L; k++) lowest = min(lowest, col[k]);
+    for (int k = 1; k + 1 < L; k += 2) lowest = __vimin3_u32(lowest, col[k], col[k + 1]);
+    lowest = min(lowest, col[L - 1]);
     const bool interrupted = (lowest == 0u);
-    const unsigned long long before = tile_checksum<L>(col);
+    const unsigned long long before = tile_checksum<L>(col, one);
     turn_maneuver<L, UP0, SOFT>(col, sw, pa, interrupted, sMD, sec, S, lane);
     if (NPASS == 2) turn_maneuver<L, !UP0, SOFT>(col, sw, pb, interrupted, sMD + S * 32, sec, S, lane);
-    if (tile_checksum<L>(col) != before) {
+    if (tile_checksum<L>(col, one) != before) {
         int row0 = sec * L;
-        asm volatile("" : "+r"(row0));        // recompute the addresses: keeping 64 of them alive across the passes spills
-#pragma unroll
-        for (int k = 0; k < L; k++) {
-            const uint2 o = soff[row0 + k];
-            V[o.x + ((o.y + lane) & mx)] = col[k];
-        }
+        asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills
+        if (!wraps) tile_rows_store<L, false>(col, V, so + row0, lane, (uint32_t)mx);
+        else tile_rows_store<L, true>(col, V, so + row0, lane, (uint32_t)mx);
     }
 }
 
@@ -348,9 +397,9 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     const TurnPass pa = pass(ma), pb = pass(mb);
     const uint8_t *Sc = left ? p->S_left : p->S_right;
     const dim3 grid(n / 32, n), block(32 * S);
-    const size_t smem = sizeof(uint2) * ((size_t)nt + 2 * (size_t)S * 32);
+    const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 2 * (size_t)S * 32;
     ProfScope prof(p, mb >= 0 ? 11 : ma);
-#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb)
+#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u)
 #define NHP_TT2(NP, UP) do { if (soft) NHP_TT(NP, UP, true); else NHP_TT(NP, UP, false); } while (0)
     if (mb >= 0) { if (up) NHP_TT2(2, true); else NHP_TT2(2, false); }
     else { if (up) NHP_TT2(1, true); else NHP_TT2(1, false); }
