@@ -207,86 +207,115 @@ __device__ __forceinline__ uint32_t sec_weight(const SecW<SOFT> &sw, const uint4
     return nhp_soft_weight(sw.len, word, K & 3);
 }
 
-template <int L, bool UP, bool SOFT, int S = 0>
+__device__ __forceinline__ void checksum_add(unsigned long long &acc, uint32_t v, uint32_t one);
+
+// Two chains per thread.  A section of L = 32 vertices is swept as two half-sections H0, H1 (in travel order) whose
+// chains are independent: both are summarised from "infinity" at the same time, the carry into H1 follows from the
+// carry into H0 and H0's summary, and both are applied at the same time.  A single chain issues one dependent
+// min/max op every ~4 cycles; two interleaved chains keep the integer pipe fed from half as many warps (the
+// Sections algebra of appendix D, one level further down).
+template <int L, bool UP, bool SOFT, bool CS, int S = 0>
 struct SecLoop {
-    static constexpr int k = UP ? S : L - 1 - S;
-    // summary pass: the section entered with "infinity" (Sv of Insert 3); t is the value AT the
+    static constexpr int H = L / 2;
+    static constexpr int ka = UP ? S : L - 1 - S;             // vertex S of H0
+    static constexpr int kb = UP ? H + S : H - 1 - S;         // vertex S of H1
+    // summary pass: each half entered with "infinity" (Sv of Insert 3); t is the value AT the
     // vertex before its own edge (nhp_arrive / nhp_gate), wp the pending weight of the vertex behind it; for soft
-    // weights d sums the edge costs across the section (Sd)
-    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t &t, uint32_t &wp, uint32_t &d)
+    // weights d sums the edge costs across the half (Sd)
+    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 qa, uint4 qb, uint32_t &ta,
+                                                   uint32_t &wa, uint32_t &da, uint32_t &tb, uint32_t &wb, uint32_t &db,
+                                                   unsigned long long &acc, uint32_t one)
     {
-        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
-        const uint32_t u = col[k];
-        t = nhp_gate(nhp_arrive(t, wp, u), u);
-        wp = sec_weight<SOFT, k>(sw, q);
-        if (SOFT) d += wp;
-        SecLoop<L, UP, SOFT, S + 1>::summary(col, sw, q, t, wp, d);
+        if (SOFT && S == 0) { qa = ld_s16(sw.sp + (ka >> 4)); qb = ld_s16(sw.sp + (kb >> 4)); }
+        const uint32_t ua = col[ka], ub = col[kb];
+        if (CS) { checksum_add(acc, ua, one); checksum_add(acc, ub, one); }
+        ta = nhp_gate(nhp_arrive(ta, wa, ua), ua);
+        tb = nhp_gate(nhp_arrive(tb, wb, ub), ub);
+        wa = sec_weight<SOFT, ka>(sw, qa);
+        wb = sec_weight<SOFT, kb>(sw, qb);
+        if (SOFT) { da += wa; db += wb; }
+        SecLoop<L, UP, SOFT, CS, S + 1>::summary(col, sw, qa, qb, ta, wa, da, tb, wb, db, acc, one);
     }
     // apply pass: the vertex keeps min(v, u), then the same step
-    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 q, uint32_t ct, uint32_t &t, uint32_t &wp)
+    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 qa, uint4 qb, uint32_t ct, uint32_t &ta,
+                                                 uint32_t &wa, uint32_t &tb, uint32_t &wb, unsigned long long &acc, uint32_t one)
     {
-        if (SOFT && (S & 15) == 0) q = ld_s16(sw.sp + (k >> 4));
-        const uint32_t u = col[k];
-        t = nhp_arrive(t, (!SOFT && S == 0) ? 0u : wp, u);
-        col[k] = nhp_keep(t, ct, u);
-        t = nhp_gate(t, u);
-        if (SOFT) wp = sec_weight<SOFT, k>(sw, q);
-        SecLoop<L, UP, SOFT, S + 1>::apply(col, sw, q, ct, t, wp);
+        if (SOFT && S == 0) { qa = ld_s16(sw.sp + (ka >> 4)); qb = ld_s16(sw.sp + (kb >> 4)); }
+        const uint32_t ua = col[ka], ub = col[kb];
+        ta = nhp_arrive(ta, (!SOFT && S == 0) ? 0u : wa, ua);
+        tb = nhp_arrive(tb, (!SOFT && S == 0) ? 0u : wb, ub);
+        col[ka] = nhp_keep(ta, ct, ua);
+        col[kb] = nhp_keep(tb, ct, ub);
+        if (CS) { checksum_add(acc, col[ka], one); checksum_add(acc, col[kb], one); }
+        ta = nhp_gate(ta, ua);
+        tb = nhp_gate(tb, ub);
+        if (SOFT) { wa = sec_weight<SOFT, ka>(sw, qa); wb = sec_weight<SOFT, kb>(sw, qb); }
+        SecLoop<L, UP, SOFT, CS, S + 1>::apply(col, sw, qa, qb, ct, ta, wa, tb, wb, acc, one);
     }
 };
-template <int L, bool UP, bool SOFT>
-struct SecLoop<L, UP, SOFT, L> {
-    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t &, uint32_t &, uint32_t &) {}
-    static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint32_t, uint32_t &, uint32_t &) {}
+template <int L, bool UP, bool SOFT, bool CS>
+struct SecLoop<L, UP, SOFT, CS, L / 2> {
+    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint4, uint32_t &, uint32_t &, uint32_t &,
+                                                   uint32_t &, uint32_t &, uint32_t &, unsigned long long &, uint32_t) {}
+    static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint4, uint32_t, uint32_t &, uint32_t &, uint32_t &,
+                                                 uint32_t &, unsigned long long &, uint32_t) {}
 };
 
 // carry into section `sec` of a closed curve cut into S (a power of two) sections, travel direction UP
 // (sec -> sec+1) or down: fold the other sections once around the curve, starting from section sec itself.
-// M <= 2^31 - 1 and D <= 2^31, so c + D never wraps.
+// The (M, D) table is stored twice, [2 S][32], so that the walk around the ring is a plain stride (one LDS with
+// an immediate offset and one DPX op per section).  M <= 2^31 - 1 and D <= 2^31, so c + D never wraps.
 template <bool UP>
 __device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int S, int lane)
 {
-    uint32_t c = sMD[sec * 32 + lane].x;
-#pragma unroll 4
+    const uint2 *q = sMD + (UP ? sec : sec + S) * 32 + lane;
+    uint32_t c = q->x;
+#pragma unroll 8
     for (int r = 1; r < S; r++) {
-        const uint2 md = sMD[((UP ? sec + r : sec - r) & (S - 1)) * 32 + lane];
+        q += UP ? 32 : -32;
+        const uint2 md = *q;
         c = __viaddmin_u32(c, md.y, md.x);
     }
     return c;
 }
 
-// 64-bit checksum sum(col): the sums before and after the passes differ iff a vertex improved (values only
-// decrease).  mad.wide runs on the FMA pipe, which the sweeps leave idle; the min/max pipe is the busy one.  The
-// multiplier 1 comes from the kernel parameters: ptxas turns a multiplication by a KNOWN 1 into ALU-pipe
-// IADD3 / IADD3.X pairs.
-template <int L>
-__device__ __forceinline__ unsigned long long tile_checksum(const uint32_t (&col)[L], uint32_t one)
+// Exact change detection: the 64-bit sums of a thread's 32 vertices before and after the passes differ iff a vertex
+// improved (values only decrease).  The additions are IMAD.WIDE on the FMA pipe and sit INSIDE the first summary
+// loop and the last apply loop, in the issue slots the min/max pipe leaves free (it takes one warp instruction every
+// other cycle); as two loops of their own they cost as much time as the chains.  The multiplier 1 comes from the
+// kernel parameters: ptxas turns a multiplication by a KNOWN 1 into ALU-pipe IADD3 / IADD3.X pairs.
+__device__ __forceinline__ void checksum_add(unsigned long long &acc, uint32_t v, uint32_t one)
 {
-    unsigned long long acc = 0;
-#pragma unroll
-    for (int k = 0; k < L; k++) asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(col[k]), "r"(one));
-    return acc;
+    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(v), "r"(one));
 }
 
 struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4 (soft)
 
-// One maneuver over the tile.  All values travel as a = v - ct (nhp_arrive): the section summary M is the value
-// arriving at the first vertex of the NEXT section, D the summed edge cost across the section.
-template <int L, bool UP, bool SOFT>
-__device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool interrupted, uint2 *sMD,
-                                              int sec, int S, int lane)
+// One maneuver over the tile.  All values travel as a = v - ct (nhp_arrive): a summary M is the value arriving at
+// the first vertex BEHIND the (half-)section, D the summed edge cost across it (>= D_CAP: a blocked vertex interrupts it).
+template <int L, bool UP, bool SOFT, bool CS_BEFORE, bool CS_AFTER>
+__device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
+                                              uint2 *sMD, int sec, int S, int lane, unsigned long long &before, unsigned long long &after,
+                                              uint32_t one)
 {
+    const bool ia = UP ? blocked_lo : blocked_hi, ib = UP ? blocked_hi : blocked_lo;     // H0, H1 in travel order
     sw.len = pass.w;
-    uint32_t t = VI_INF, wp = SOFT ? 0u : pass.w, d = 0;
-    SecLoop<L, UP, SOFT>::summary(col, sw, make_uint4(0, 0, 0, 0), t, wp, d);
-    if (!SOFT) d = (uint32_t)L * pass.w;
-    sMD[sec * 32 + lane] = make_uint2(__viaddmin_u32(t, wp, 0x7fffffffu), interrupted ? D_CAP : d);
+    uint32_t ta = VI_INF, tb = VI_INF, wa = SOFT ? 0u : pass.w, wb = wa, da = 0, db = 0;
+    SecLoop<L, UP, SOFT, CS_BEFORE>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, before, one);
+    if (!SOFT) da = db = (uint32_t)(L / 2) * pass.w;
+    const uint32_t ma = __viaddmin_u32(ta, wa, 0x7fffffffu), mb = __viaddmin_u32(tb, wb, 0x7fffffffu);
+    const uint32_t Da = ia ? D_CAP : da;
+    // section = H0 then H1: (Da, ma) o (Db, mb) = (Da + Db, min(ma + Db, mb)), Insert 4 PAPER.md:935-939
+    const uint2 md = make_uint2(__viaddmin_u32(ma, ib ? D_CAP : db, mb), (ia || ib) ? D_CAP : da + db);
+    sMD[sec * 32 + lane] = md;
+    sMD[(sec + S) * 32 + lane] = md;
     __syncthreads();
-    t = ripple_carry<UP>(sMD, sec, S, lane);
+    ta = ripple_carry<UP>(sMD, sec, S, lane);                 // carry into H0
+    tb = __viaddmin_u32(ta, Da, ma);                          // carry into H1: through H0, or from inside it
     // opaque copy of the weight: otherwise the per-vertex values of the summary pass are kept alive for the apply pass
     asm volatile("" : "+r"(sw.len));
-    wp = SOFT ? 0u : sw.len;
-    SecLoop<L, UP, SOFT>::apply(col, sw, make_uint4(0, 0, 0, 0), pass.ct, t, wp);
+    wa = wb = SOFT ? 0u : sw.len;
+    SecLoop<L, UP, SOFT, CS_AFTER>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
 }
 
 // Row addressing of a tile: so[t] = element index of the tile's first vertex in plane t (row base + first column).
@@ -338,7 +367,7 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     extern __shared__ __align__(16) uint32_t smem[];
     const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
     uint32_t *so = smem;                                      // [nt] element index of the tile's first vertex in every plane
-    uint2 *sMD = (uint2 *)(so + nt);                          // [2][S][32] (M, D) of every section, one set per maneuver
+    uint2 *sMD = (uint2 *)(so + nt);                          // [2][2 S][32] (M, D) of every section (twice), one set per maneuver
     const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
     int seam = 0;
@@ -355,16 +384,18 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     uint32_t col[L];
     if (!wraps) tile_rows_load<L, false>(col, V, so + sec * L, lane, (uint32_t)mx);
     else tile_rows_load<L, true>(col, V, so + sec * L, lane, (uint32_t)mx);
-    // blocked vertices never change, so "does a blocked vertex interrupt my section" is decided once
-    uint32_t lowest = col[0];
+    // blocked vertices never change, so "does a blocked vertex interrupt this half of my section" is decided once
+    uint32_t lo = col[0], hi = col[L / 2];
 #pragma unroll
-    for (int k = 1; k + 1 < L; k += 2) lowest = __vimin3_u32(lowest, col[k], col[k + 1]);
-    lowest = min(lowest, col[L - 1]);
-    const bool interrupted = (lowest == 0u);
-    const unsigned long long before = tile_checksum<L>(col, one);
-    turn_maneuver<L, UP0, SOFT>(col, sw, pa, interrupted, sMD, sec, S, lane);
-    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT>(col, sw, pb, interrupted, sMD + S * 32, sec, S, lane);
-    if (tile_checksum<L>(col, one) != before) {
+    for (int k = 1; k + 1 < L / 2; k += 2) {
+        lo = __vimin3_u32(lo, col[k], col[k + 1]);
+        hi = __vimin3_u32(hi, col[L / 2 + k], col[L / 2 + k + 1]);
+    }
+    const bool blocked_lo = min(lo, col[L / 2 - 1]) == 0u, blocked_hi = min(hi, col[L - 1]) == 0u;
+    unsigned long long before = 0, after = 0;
+    turn_maneuver<L, UP0, SOFT, true, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, sMD, sec, S, lane, before, after, one);
+    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT, false, true>(col, sw, pb, blocked_lo, blocked_hi, sMD + 2 * S * 32, sec, S, lane, before, after, one);
+    if (after != before) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills
         if (!wraps) tile_rows_store<L, false>(col, V, so + row0, lane, (uint32_t)mx);
@@ -397,7 +428,7 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     const TurnPass pa = pass(ma), pb = pass(mb);
     const uint8_t *Sc = left ? p->S_left : p->S_right;
     const dim3 grid(n / 32, n), block(32 * S);
-    const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 2 * (size_t)S * 32;
+    const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 4 * (size_t)S * 32;
     ProfScope prof(p, mb >= 0 ? 11 : ma);
 #define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u)
 #define NHP_TT2(NP, UP) do { if (soft) NHP_TT(NP, UP, true); else NHP_TT(NP, UP, false); } while (0)
