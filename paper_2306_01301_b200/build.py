@@ -27,7 +27,7 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc] + NVCC_FLAGS + ["-o", LIB] + sources()
+        cmd = [nvcc] + NVCC_FLAGS + os.environ.get("NHP_NVCC_EXTRA", "").split() + ["-o", LIB] + sources()
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode != 0:
             print(r.stdout)

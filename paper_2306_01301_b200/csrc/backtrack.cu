@@ -76,10 +76,8 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
             }
             const int maxk = turn ? nt - 1 : n;
             const uint32_t ct = P.ct[m];
-            unsigned long long E = 0;
-            for (int base = 0; base < maxk; base += 32) {
-                const int k = base + lane + 1;                 // steps back, against the direction of m
-                int i, j, t;
+            // vertex k steps back, against the direction of m
+            auto cell = [&](int k, int &i, int &j, int &t) {
                 if (turn) {
                     t = (up ? cth - k : cth + k) & mt;
                     i = (xp + T.beta[(t + qa * quarter) & mt]) & mx;
@@ -89,39 +87,55 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
                     const int c = (xp + Bt[y]) & mx;
                     t = cth; i = I ? c : y; j = I ? y : c;
                 }
-                const size_t idx = ((((size_t)t << log2_n) + j) << log2_n) + i;
-                const bool valid = k <= maxk;
-                const uint32_t u = valid ? V[idx] : 0u;
-                const unsigned blk = __ballot_sync(0xffffffffu, u == 0u);       // blocked (or past the end)
-                const int first = blk ? __ffs(blk) - 1 : 32;
-                uint32_t w = T.len_q[(size_t)m * nt + t];
-                if (P.soft) w = (w * (uint32_t)(valid ? S[idx] : 16)) >> 4;
-                unsigned long long pre = (lane < first) ? w : 0;                 // inclusive prefix sum of w
+            };
+            unsigned long long E = 0;
+            bool done = false;
+            constexpr int NB = 8;                              // chunks of 32 vertices whose loads are in flight together
+            for (int base = 0; base < maxk && !done; base += 32 * NB) {
+                uint32_t uu[NB], ww[NB];
 #pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const unsigned long long y = __shfl_up_sync(0xffffffffu, pre, d);
-                    if (lane >= d) pre += y;
+                for (int c = 0; c < NB; c++) {
+                    const int k = base + 32 * c + lane + 1;
+                    int i, j, t;
+                    cell(k, i, j, t);
+                    const size_t idx = ((((size_t)t << log2_n) + j) << log2_n) + i;
+                    const bool valid = k <= maxk;
+                    uu[c] = valid ? V[idx] : 0u;
+                    uint32_t w = T.len_q[(size_t)m * nt + t];
+                    if (P.soft) w = (w * (uint32_t)(valid ? S[idx] : 16)) >> 4;
+                    ww[c] = w;
                 }
-                pre += E;
-                unsigned long long key = KINF;
-                uint32_t seg = 0;
-                if (lane < first && u < VI_INF) {
-                    const unsigned long long cand = (unsigned long long)(u - 1u) + ct + pre;
-                    if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ct + pre); }
+#pragma unroll
+                for (int c = 0; c < NB; c++) {
+                    if (done) continue;                          // warp-uniform
+                    const int k = base + 32 * c + lane + 1;
+                    const uint32_t u = uu[c];
+                    const unsigned blk = __ballot_sync(0xffffffffu, u == 0u);       // blocked (or past the end)
+                    const int first = blk ? __ffs(blk) - 1 : 32;
+                    unsigned long long pre = (lane < first) ? ww[c] : 0;             // inclusive prefix sum of w
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const unsigned long long y = __shfl_up_sync(0xffffffffu, pre, d);
+                        if (lane >= d) pre += y;
+                    }
+                    pre += E;
+                    unsigned long long key = KINF;
+                    uint32_t seg = 0;
+                    if (lane < first && u < VI_INF) {
+                        const unsigned long long cand = (unsigned long long)(u - 1u) + ct + pre;
+                        if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ct + pre); }
+                    }
+                    const unsigned long long kmin = warp_min_u64(key);
+                    if (kmin < best) {                               // strictly smaller: earlier chunks win ties
+                        best = kmin;
+                        const unsigned who = __ballot_sync(0xffffffffu, key == kmin);
+                        best_seg = __shfl_sync(0xffffffffu, seg, __ffs(who) - 1);
+                    }
+                    E = __shfl_sync(0xffffffffu, pre, 31);
+                    if (first < 32) done = true;
                 }
-                const unsigned long long kmin = warp_min_u64(key);
-                if (kmin < best) {                               // strictly smaller: earlier chunks win ties
-                    best = kmin;
-                    const unsigned who = __ballot_sync(0xffffffffu, key == kmin);
-                    const int src = __ffs(who) - 1;
-                    best_seg = __shfl_sync(0xffffffffu, seg, src);
-                    bi = __shfl_sync(0xffffffffu, i, src);
-                    bj = __shfl_sync(0xffffffffu, j, src);
-                    bt = __shfl_sync(0xffffffffu, t, src);
-                }
-                E = __shfl_sync(0xffffffffu, pre, 31);
-                if (first < 32) break;
             }
+            if (best != KINF) cell((int)(best & 0x1fffu), bi, bj, bt);
         }
         if (lane == 0) { s_key[m] = best; s_seg[m] = best_seg; s_cell[m][0] = bi; s_cell[m][1] = bj; s_cell[m][2] = bt; }
         __syncthreads();
