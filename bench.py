@@ -208,6 +208,12 @@ def run_ours(args):
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
     traffic = measured_traffic(args.config, dom)
+    # secondary bound: the integer min/max pipe, 16 lanes per SM sub-partition and clock
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_clock = (clk or {}).get("sm_mhz") or 1965.0
+    alu_peak = sm_count * 4 * 16 * sm_clock * 1e6 / 1e12                       # T lane-ops / s
+    ops_per_update = 3 if dom in ("SF", "SB") else 5
+    alu_achieved = ops_per_update * n_r * (2 if dom == "turn_pair" else 1) / (dom_ms / max(dom_n, 1) * 1e-3) / 1e12 if dom_ms > 0 else 0.0
     out = {
         "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
@@ -228,6 +234,9 @@ def run_ours(args):
                      "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
                      "launches_timed": int(dom_n),
                      "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
+        "alu": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": alu_peak, "unit": "T min/max lane-ops/s",
+                "frac": alu_achieved / alu_peak, "ops_per_pose_update": ops_per_update,
+                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.5)"},
         "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
     }
     if not args.no_cpu_baseline and ws == 1:

@@ -214,7 +214,7 @@ __device__ __forceinline__ void checksum_add(unsigned long long &acc, uint32_t v
 // carry into H0 and H0's summary, and both are applied at the same time.  A single chain issues one dependent
 // min/max op every ~4 cycles; two interleaved chains keep the integer pipe fed from half as many warps (the
 // Sections algebra of appendix D, one level further down).
-template <int L, bool UP, bool SOFT, bool CS, int S = 0>
+template <int L, bool UP, bool SOFT, bool CS, bool GATE, int S = 0>
 struct SecLoop {
     static constexpr int H = L / 2;
     static constexpr int ka = UP ? S : L - 1 - S;             // vertex S of H0
@@ -229,12 +229,13 @@ struct SecLoop {
         if (SOFT && S == 0) { qa = ld_s16(sw.sp + (ka >> 4)); qb = ld_s16(sw.sp + (kb >> 4)); }
         const uint32_t ua = col[ka], ub = col[kb];
         if (CS) { checksum_add(acc, ua, one); checksum_add(acc, ub, one); }
-        ta = nhp_gate(nhp_arrive(ta, wa, ua), ua);
-        tb = nhp_gate(nhp_arrive(tb, wb, ub), ub);
+        ta = nhp_arrive(ta, wa, ua);
+        tb = nhp_arrive(tb, wb, ub);
+        if (GATE) { ta = nhp_gate(ta, ua); tb = nhp_gate(tb, ub); }
         wa = sec_weight<SOFT, ka>(sw, qa);
         wb = sec_weight<SOFT, kb>(sw, qb);
         if (SOFT) { da += wa; db += wb; }
-        SecLoop<L, UP, SOFT, CS, S + 1>::summary(col, sw, qa, qb, ta, wa, da, tb, wb, db, acc, one);
+        SecLoop<L, UP, SOFT, CS, GATE, S + 1>::summary(col, sw, qa, qb, ta, wa, da, tb, wb, db, acc, one);
     }
     // apply pass: the vertex keeps min(v, u), then the same step
     static __device__ __forceinline__ void apply(uint32_t (&col)[L], const SecW<SOFT> &sw, uint4 qa, uint4 qb, uint32_t ct, uint32_t &ta,
@@ -247,14 +248,13 @@ struct SecLoop {
         col[ka] = nhp_keep(ta, ct, ua);
         col[kb] = nhp_keep(tb, ct, ub);
         if (CS) { checksum_add(acc, col[ka], one); checksum_add(acc, col[kb], one); }
-        ta = nhp_gate(ta, ua);
-        tb = nhp_gate(tb, ub);
+        if (GATE) { ta = nhp_gate(ta, ua); tb = nhp_gate(tb, ub); }
         if (SOFT) { wa = sec_weight<SOFT, ka>(sw, qa); wb = sec_weight<SOFT, kb>(sw, qb); }
-        SecLoop<L, UP, SOFT, CS, S + 1>::apply(col, sw, qa, qb, ct, ta, wa, tb, wb, acc, one);
+        SecLoop<L, UP, SOFT, CS, GATE, S + 1>::apply(col, sw, qa, qb, ct, ta, wa, tb, wb, acc, one);
     }
 };
-template <int L, bool UP, bool SOFT, bool CS>
-struct SecLoop<L, UP, SOFT, CS, L / 2> {
+template <int L, bool UP, bool SOFT, bool CS, bool GATE>
+struct SecLoop<L, UP, SOFT, CS, GATE, L / 2> {
     static __device__ __forceinline__ void summary(const uint32_t (&)[L], const SecW<SOFT> &, uint4, uint4, uint32_t &, uint32_t &, uint32_t &,
                                                    uint32_t &, uint32_t &, uint32_t &, unsigned long long &, uint32_t) {}
     static __device__ __forceinline__ void apply(uint32_t (&)[L], const SecW<SOFT> &, uint4, uint4, uint32_t, uint32_t &, uint32_t &, uint32_t &,
@@ -280,9 +280,9 @@ __device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int 
 }
 
 // Exact change detection: the 64-bit sums of a thread's 32 vertices before and after the passes differ iff a vertex
-// improved (values only decrease).  The additions are IMAD.WIDE on the FMA pipe and sit INSIDE the first summary
-// loop and the last apply loop, in the issue slots the min/max pipe leaves free (it takes one warp instruction every
-// other cycle); as two loops of their own they cost as much time as the chains.  The multiplier 1 comes from the
+// improved (values only decrease).  The additions are IMAD.WIDE on the FMA pipe; the "after" sum sits INSIDE the last
+// apply loop, in the issue slots the min/max pipe leaves free (it takes one warp instruction every other cycle); the
+// "before" sum is taken up front because it also tells whether every vertex of the warp is blocked.  The multiplier 1 comes from the
 // kernel parameters: ptxas turns a multiplication by a KNOWN 1 into ALU-pipe IADD3 / IADD3.X pairs.
 __device__ __forceinline__ void checksum_add(unsigned long long &acc, uint32_t v, uint32_t one)
 {
@@ -293,15 +293,29 @@ struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4
 
 // One maneuver over the tile.  All values travel as a = v - ct (nhp_arrive): a summary M is the value arriving at
 // the first vertex BEHIND the (half-)section, D the summed edge cost across it (>= D_CAP: a blocked vertex interrupts it).
-template <int L, bool UP, bool SOFT, bool CS_BEFORE, bool CS_AFTER>
+// Two warp-uniform short cuts (the only data-dependent control flow of the sweeps; the result is the same):
+//   all_blocked   every vertex of the warp's 32 curves x 32 planes is blocked (deep inside an obstacle of the
+//                 configuration space, ~20 % of the warps in configs 3 and 4): the section passes nothing on
+//                 (M = infinity, D = D_CAP) and has nothing to update
+//   none_blocked  no vertex is blocked (~16 %): the chains run without the nhp_gate op
+template <int L, bool UP, bool SOFT, bool CS_AFTER>
 __device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
-                                              uint2 *sMD, int sec, int S, int lane, unsigned long long &before, unsigned long long &after,
-                                              uint32_t one)
+                                              bool all_blocked, bool none_blocked, uint2 *sMD, int sec, int S, int lane,
+                                              unsigned long long &after, uint32_t one)
 {
+    if (all_blocked) {
+        const uint2 md = make_uint2(0x7fffffffu, D_CAP);
+        sMD[sec * 32 + lane] = md;
+        sMD[(sec + S) * 32 + lane] = md;
+        __syncthreads();
+        return;
+    }
     const bool ia = UP ? blocked_lo : blocked_hi, ib = UP ? blocked_hi : blocked_lo;     // H0, H1 in travel order
     sw.len = pass.w;
     uint32_t ta = VI_INF, tb = VI_INF, wa = SOFT ? 0u : pass.w, wb = wa, da = 0, db = 0;
-    SecLoop<L, UP, SOFT, CS_BEFORE>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, before, one);
+    unsigned long long unused = 0;
+    if (none_blocked) SecLoop<L, UP, SOFT, false, false>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, unused, one);
+    else SecLoop<L, UP, SOFT, false, true>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, unused, one);
     if (!SOFT) da = db = (uint32_t)(L / 2) * pass.w;
     const uint32_t ma = __viaddmin_u32(ta, wa, 0x7fffffffu), mb = __viaddmin_u32(tb, wb, 0x7fffffffu);
     const uint32_t Da = ia ? D_CAP : da;
@@ -315,7 +329,8 @@ __device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
     // opaque copy of the weight: otherwise the per-vertex values of the summary pass are kept alive for the apply pass
     asm volatile("" : "+r"(sw.len));
     wa = wb = SOFT ? 0u : sw.len;
-    SecLoop<L, UP, SOFT, CS_AFTER>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
+    if (none_blocked) SecLoop<L, UP, SOFT, CS_AFTER, false>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
+    else SecLoop<L, UP, SOFT, CS_AFTER, true>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
 }
 
 // Row addressing of a tile: so[t] = element index of the tile's first vertex in plane t (row base + first column).
@@ -393,8 +408,14 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     }
     const bool blocked_lo = min(lo, col[L / 2 - 1]) == 0u, blocked_hi = min(hi, col[L - 1]) == 0u;
     unsigned long long before = 0, after = 0;
-    turn_maneuver<L, UP0, SOFT, true, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, sMD, sec, S, lane, before, after, one);
-    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT, false, true>(col, sw, pb, blocked_lo, blocked_hi, sMD + 2 * S * 32, sec, S, lane, before, after, one);
+#pragma unroll
+    for (int k = 0; k < L; k++) checksum_add(before, col[k], one);
+    const bool all_blocked = __all_sync(0xffffffffu, before == 0ull);
+    // (soft kernels keep one chain variant: a second copy of their loops costs registers they do not have)
+    const bool none_blocked = !SOFT && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
+    turn_maneuver<L, UP0, SOFT, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, sMD, sec, S, lane, after, one);
+    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, sMD + 2 * S * 32, sec, S, lane, after, one);
+    if (all_blocked) after = before;
     if (after != before) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills

@@ -34,6 +34,9 @@ def small_scenes():
         scenes.random_scene(6, 6, 8, 5, flags=1, soft=True),                       # forward only
         scenes.random_scene(5, 7, 4, 6, ct=(4096, 0, 5000, 5000, 0, 4096)),        # N_theta > N, compact weights
         scenes.random_scene(7, 6, 9, 7, vehicle=(9, 4), n_rects=20, soft=True, reverse_mult=300, n_cycles=2),
+        scenes.random_scene(5, 10, 6, 8, n_cycles=2),                                # N_theta = 1024: 32 sections, 1024-thread tiles
+        scenes.random_scene(5, 10, 5, 9, soft=True, reverse_mult=400, n_cycles=2),
+        scenes.random_scene(8, 5, 4.5, 10, vehicle=(3, 2), n_rects=40, n_cycles=2),  # N = 256, N_theta = 32: one section per curve
     ]
 
 
