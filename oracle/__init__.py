@@ -246,3 +246,36 @@ class Oracle:
         if rc:
             raise OracleError(rc, "backtrack")
         return [(w.i, w.j, w.theta, w.m) for w in out[:cnt.value]], cost.value
+
+
+def soft_from_hard(hard: np.ndarray, k: float = 4.0):
+    """Steps 1-2 of PAPER.md:388-389 under reading DESIGN R17: exact squared distance transform of hard | wall,
+    float32 distance, Q4.4 soft image.  Returns (d2 int32, dist float32, soft uint8)."""
+    L = _load_dt()
+    h = np.ascontiguousarray(hard, np.uint8)
+    n = h.shape[0]
+    d2 = np.empty((n, n), np.int32); dist = np.empty((n, n), np.float32); soft = np.empty((n, n), np.uint8)
+    rc = L.orc_soft_from_hard(h.ctypes.data_as(C.c_void_p), n, C.c_float(k), d2.ctypes.data_as(C.c_void_p),
+                              dist.ctypes.data_as(C.c_void_p), soft.ctypes.data_as(C.c_void_p))
+    assert rc == 0
+    return d2, dist, soft
+
+
+def edt_brute(hard: np.ndarray) -> np.ndarray:
+    """Squared distance to the nearest pixel of hard | wall by the O(N^4) definition (tiny images only)."""
+    L = _load_dt()
+    h = np.ascontiguousarray(hard, np.uint8)
+    n = h.shape[0]
+    d2 = np.empty((n, n), np.int32)
+    L.orc_edt_brute(h.ctypes.data_as(C.c_void_p), n, d2.ctypes.data_as(C.c_void_p))
+    return d2
+
+
+def _load_dt():
+    build()
+    L = C.CDLL(_LIB)
+    L.orc_soft_from_hard.restype = C.c_int
+    L.orc_soft_from_hard.argtypes = [C.c_void_p, C.c_int, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.orc_edt_brute.restype = None
+    L.orc_edt_brute.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+    return L

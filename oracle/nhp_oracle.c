@@ -626,3 +626,72 @@ int orc_backtrack(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const u
     *count = cnt; *cost = total;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Steps 1-2 of the pipeline (section VII l.342): "distance transform obstacle image
+ * and calculate new obstacle image as a function of distance".  The paper leaves the function open
+ * ("some function of the distance"); reading DESIGN R17:
+ *     H     = hard | wall (row 0 and column 0), NOT toroidal (as the scene generators do)
+ *     d2    = exact squared Euclidean distance of a pixel centre to the nearest pixel centre of H
+ *     d     = sqrtf(d2)                                   float32, correctly rounded
+ *     soft  = clamp(rintf(16 * (1 + k / (d + 1))), 16, 255)  float32 operation by operation (no FMA), Q4.4
+ * Plain definition written out: for every pixel the minimum over ALL hard pixels (orc_edt_brute, O(N^4),
+ * tiny images only), and the exact separable form min over x' of (x - x')^2 + g(y, x')^2 with g = distance
+ * to the nearest hard pixel in column x' (orc_soft_from_hard, O(N^3)).  Pins: the two agree; both agree
+ * with scipy.ndimage.distance_transform_edt (tests/test_oracle_dt.py).
+ * ------------------------------------------------------------------------------------------------ */
+#define ORC_DT_FAR 20000            /* "no hard pixel in this column": FAR^2 + N^2 < 2^31 for N <= 4096 */
+
+static int dt_hard(const uint8_t *hard, int n, int x, int y) { return hard[(size_t)y * n + x] != 0 || x == 0 || y == 0; }
+
+void orc_edt_brute(const uint8_t *hard, int n, int32_t *d2_out)
+{
+    for (int y = 0; y < n; y++)
+        for (int x = 0; x < n; x++) {
+            int64_t best = INT64_MAX;
+            for (int b = 0; b < n; b++)
+                for (int a = 0; a < n; a++)
+                    if (dt_hard(hard, n, a, b)) {
+                        int64_t d = (int64_t)(x - a) * (x - a) + (int64_t)(y - b) * (y - b);
+                        if (d < best) best = d;
+                    }
+            d2_out[(size_t)y * n + x] = (int32_t)best;
+        }
+}
+
+/* d2_out (int32, may be NULL), dist_out (float, may be NULL), soft_out (uint8, may be NULL): n x n each */
+int orc_soft_from_hard(const uint8_t *hard, int n, float k, int32_t *d2_out, float *dist_out, uint8_t *soft_out)
+{
+    int32_t *g = (int32_t *)malloc(sizeof(int32_t) * (size_t)n * n);
+    if (!g) return -1;
+    for (int x = 0; x < n; x++) {                      /* nearest hard pixel in the same column */
+        for (int y = 0; y < n; y++) {
+            int best = ORC_DT_FAR;
+            for (int b = 0; b < n; b++)
+                if (dt_hard(hard, n, x, b)) { int d = y > b ? y - b : b - y; if (d < best) best = d; }
+            g[(size_t)y * n + x] = best;
+        }
+    }
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < n; y++)
+        for (int x = 0; x < n; x++) {
+            int64_t best = INT64_MAX;
+            for (int a = 0; a < n; a++) {
+                int64_t gg = g[(size_t)y * n + a];
+                int64_t d = (int64_t)(x - a) * (x - a) + gg * gg;
+                if (d < best) best = d;
+            }
+            const size_t idx = (size_t)y * n + x;
+            if (d2_out) d2_out[idx] = (int32_t)best;
+            volatile float d = sqrtf((float)best);     /* volatile: one rounding per operation, no contraction */
+            volatile float den = d + 1.0f;
+            volatile float q = k / den;
+            volatile float s = 1.0f + q;
+            volatile float v = 16.0f * s;
+            float r = rintf(v);
+            if (dist_out) dist_out[idx] = d;
+            if (soft_out) soft_out[idx] = (uint8_t)(r < 16.0f ? 16.0f : r > 255.0f ? 255.0f : r);
+        }
+    free(g);
+    return 0;
+}
