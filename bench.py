@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--cycles", type=int, default=0, help="override N_T (0 = the config's own)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--simple-kernels", action="store_true", help="thread-per-curve bring-up kernels (A/B)")
+    ap.add_argument("--dt-on-device", action="store_true",
+                    help="soft configs: distance transform + soft image on the GPU (nhp_render_obstacles_dt) instead of the harness image")
     return ap.parse_args()
 
 
@@ -152,8 +154,13 @@ def run_ours(args):
     soft_h = torch.from_numpy(sc.soft).pin_memory() if sc.soft is not None else None
     state = {"goal": tuple(sc.goal), "plan": None}
 
+    dt_dev = args.dt_on_device and sc.soft is not None
+
     def step(hard, soft):
-        p.render_obstacles(hard, soft)
+        if dt_dev:
+            p.render_obstacles_dt(hard, 4.0)                       # pipeline steps 1-4 on the device
+        else:
+            p.render_obstacles(hard, soft)
         p.run_nturn(sc.start, n_cycles)
         try:
             state["plan"] = p.extract_path(state["goal"])          # synchronises; plan comes back to the host
@@ -186,7 +193,10 @@ def run_ours(args):
     clocks = ClockSampler(local_rank)
     if rank == 0:
         clocks.start()
-    ms_dev, launches = timed(hard_d, soft_d, True)
+    ms_dev, launches = timed(hard_d, soft_d, False)
+    # the same K steps once more with an event pair around every launch: per-kernel durations for the roofline lines
+    # (the events cost ~3 % of the step, so `value` is taken from the pass without them)
+    ms_prof, _ = timed(hard_d, soft_d, True)
     kt = p.kernel_times(reset=True)
     clk = clocks.stop() if rank == 0 else None
     ms_e2e, _ = timed(hard_h, soft_h, False)
@@ -208,7 +218,7 @@ def run_ours(args):
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
     traffic = measured_traffic(args.config, dom)
-    # secondary bound (DESIGN.md 6.5): the integer min/max pipe, 16 lanes per SM sub-partition and clock
+    # secondary bound (DESIGN.md 6.6): the integer min/max pipe, 16 lanes per SM sub-partition and clock
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     sm_clock = (clk or {}).get("sm_mhz") or 1965.0
     alu_peak = sm_count * 4 * 16 * sm_clock * 1e6 / 1e12                       # T lane-ops / s
@@ -219,13 +229,13 @@ def run_ours(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
         "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config,
-                   "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)",
+                   "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)", "soft_image": ("device distance transform" if dt_dev else "harness (CPU)") if sc.soft is not None else None,
                    "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
                    "goal": list(state["goal"]), "plan_waypoints": len(plan), "plan_cost": cost},
         "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
         "clocks": clk,
         "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
-                "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if soft_h is not None else 0)),
+                "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if (soft_h is not None and not dt_dev) else 0)),
                 "d2h_bytes_per_step": int(16 * 4096 + 32)},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": n_r * (2 if dom == "turn_pair" else 1), "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -236,8 +246,9 @@ def run_ours(args):
                      "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
         "alu": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": alu_peak, "unit": "T min/max lane-ops/s",
                 "frac": alu_achieved / alu_peak, "ops_per_pose_update": ops_per_update,
-                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.5)"},
+                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.6)"},
         "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
+        "ms_per_step_with_kernel_events": ms_prof / args.steps,
     }
     if not args.no_cpu_baseline and ws == 1:
         out["cpu_baseline"] = cpu_baseline(sc, n_cycles, sample_cycles=2)

@@ -135,6 +135,20 @@ int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int m
  * footprint, 16, 255) (DESIGN R16).  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_CUDA. */
 int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *soft, int on_device);
 
+/* Steps 1-4 of PAPER.md:388-391 with the distance transform on the DEVICE (the paper runs steps 1-2 on the CPU):
+ * the soft image is synthesised from the hard image and then rendered exactly as by nhp_render_obstacles.
+ * Reading DESIGN R17 of "some function of the distance" (section VII l.342): with H = hard | wall (row 0 and
+ * column 0, not toroidal), d = float32 sqrt of the exact squared Euclidean distance to the nearest pixel of H,
+ *     soft = clamp(rint(16 * (1 + k / (d + 1))), 16, 255)        Q4.4, float32, every operation rounded once.
+ *   hard          N x N uint8 image as for nhp_render_obstacles (HOST, or DEVICE with on_device = 1)
+ *   k             strength of the soft cost, 0 <= k <= 64 (4 in the benchmarks; 0 = no soft cost)
+ *   dist_dev_out  DEVICE array of N x N floats that receives d, or NULL
+ * Requires NHP_FLAG_SOFT.  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_CUDA. */
+int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, double k, float *dist_dev_out);
+
+/* Debug accessor: the soft image the last render used (N x N uint8) -> HOST.  Synchronises the stream. */
+int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host);
+
 /* Step 5 of PAPER.md:392: V <- INF, V[start] <- 0, then n_cycles maneuver cycles LF, SF, RB, RF, SB, LB
  * (PAPER.md:475), each an in-place min-plus sweep of every curve of that maneuver (Inserts
  * 3-5 l.922-949) gated by C and weighted by S.  n_cycles <= 0 selects the paper's default of 8.
@@ -184,8 +198,9 @@ long long nhp_launch_count(const nhp_planner *p);
  *   slots 0..5  maneuver kernels in cycle order (LF, SF, RB, RF, SB, LB)
  *   slot 6      collision rendering (a1), slot 7 soft rendering (a2), slot 8 volume init / export (a6),
  *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing,
- *   slot 11     turn-pair launches (RB+RF or LB+next LF in one kernel: two maneuvers per launch) */
-#define NHP_KERNEL_SLOTS 12
+ *   slot 11     turn-pair launches (RB+RF or LB+next LF in one kernel: two maneuvers per launch)
+ *   slot 12     distance transform + soft-image synthesis (nhp_render_obstacles_dt) */
+#define NHP_KERNEL_SLOTS 13
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
 

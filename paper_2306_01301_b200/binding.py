@@ -16,12 +16,13 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
           -5: "NHP_E_GOAL_UNREACHED", -6: "NHP_E_BUFFER", -7: "NHP_E_CUDA", -8: "NHP_E_STATE", -9: "NHP_E_WEIGHTS"}
 
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
-           "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_run_nturn", "nhp_run_more",
+           "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
+           "nhp_run_nturn", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
-KERNEL_SLOTS = 12
+KERNEL_SLOTS = 13
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
-                     "backtrack", "raster_pack", "turn_pair")
+                     "backtrack", "raster_pack", "turn_pair", "distance_transform")
 
 
 class Weights(C.Structure):
@@ -69,6 +70,8 @@ def load_library():
         L.nhp_last_error.restype = C.c_char_p
         L.nhp_render_vehicle_footprint.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double]
         L.nhp_render_obstacles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
+        L.nhp_render_obstacles_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
+        L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
         L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
         L.nhp_run_more.argtypes = [C.c_void_p, C.c_int]
         L.nhp_cost_volume.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
@@ -168,6 +171,28 @@ class Planner:
         assert soft is None or hd == sd
         self._keep = (hard, soft)                       # host buffers must outlive the async copy
         self._check(self._L.nhp_render_obstacles(self._h, hp, sp, hd), "render_obstacles")
+
+    def render_obstacles_dt(self, hard, k=4.0, dist_out=None):
+        """Distance transform + soft image on the device, then rendering (nhp_render_obstacles_dt).
+        dist_out: optional float32 CUDA tensor (N, N) that receives the distance image."""
+        if isinstance(hard, np.ndarray):
+            assert hard.dtype == np.uint8 and hard.flags.c_contiguous and hard.shape == (self.n, self.n)
+            hp, hd = hard.ctypes.data, 0
+        else:
+            assert hard.dtype == self.torch.uint8 and hard.is_contiguous() and tuple(hard.shape) == (self.n, self.n)
+            hp, hd = hard.data_ptr(), int(hard.is_cuda)
+        dp = None
+        if dist_out is not None:
+            assert dist_out.is_cuda and dist_out.dtype == self.torch.float32 and dist_out.is_contiguous()
+            assert tuple(dist_out.shape) == (self.n, self.n)
+            dp = dist_out.data_ptr()
+        self._keep = (hard, dist_out)
+        self._check(self._L.nhp_render_obstacles_dt(self._h, hp, hd, float(k), dp), "render_obstacles_dt")
+
+    def soft_image_numpy(self):
+        out = np.empty((self.n, self.n), np.uint8)
+        self._check(self._L.nhp_debug_soft_image(self._h, out.ctypes.data), "debug_soft_image")
+        return out
 
     def run_nturn(self, start, n_cycles=8):
         self._check(self._L.nhp_run_nturn(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_cycles)), "run_nturn")

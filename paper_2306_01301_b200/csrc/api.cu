@@ -161,6 +161,7 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     auto alloc = [&](void **ptr, size_t bytes) { if (rc == NHP_OK && cudaMalloc(ptr, bytes) != cudaSuccess) rc = NHP_E_CUDA; };
     alloc((void **)&p->d_hard, npx);
     alloc((void **)&p->d_soft, npx);
+    if (w->flags & NHP_FLAG_SOFT) alloc((void **)&p->d_dtg, sizeof(int32_t) * npx);
     alloc((void **)&p->d_status, sizeof(int32_t) * 8);
     alloc((void **)&p->d_plan, sizeof(nhp_waypoint) * p->plan_cap);
     if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * 8) != cudaSuccess) rc = NHP_E_CUDA;
@@ -178,7 +179,7 @@ int nhp_planner_destroy(nhp_planner *p)
     cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
     cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
     cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
-    cudaFree(p->d_status); cudaFree(p->d_plan);
+    cudaFree(p->d_status); cudaFree(p->d_plan); cudaFree(p->d_dtg);
     if (p->h_status) cudaFreeHost(p->h_status);
     if (p->h_plan) cudaFreeHost(p->h_plan);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
@@ -230,6 +231,32 @@ int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *sof
     CU(cudaGetLastError());
     p->have_render = true;
     p->have_run = false;
+    return NHP_OK;
+}
+
+int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, double k, float *dist_dev_out)
+{
+    if (!p || !hard) return fail(p, NHP_E_ARG, "hard image is NULL");
+    if (!(k >= 0.0) || k > 64.0) return fail(p, NHP_E_ARG, "k outside [0, 64]");
+    if (!p->have_footprint) return fail(p, NHP_E_STATE, "render_obstacles before render_vehicle_footprint");
+    if (!p->S || !p->d_dtg) return fail(p, NHP_E_ARG, "the planner has no soft volume (NHP_FLAG_SOFT)");
+    const size_t npx = (size_t)p->n * p->n;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(p->d_hard, hard, npx, kind, p->stream));
+    p->launches += launch_soft_from_hard(p, (float)k, dist_dev_out, nullptr);        // steps 1-2
+    p->launches += launch_render(p, true);                                            // step 4
+    CU(cudaGetLastError());
+    p->have_render = true;
+    p->have_run = false;
+    return NHP_OK;
+}
+
+int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host)
+{
+    if (!p || !soft_host) return fail(p, NHP_E_ARG, "NULL argument");
+    if (!p->S || !p->have_render) return fail(p, NHP_E_STATE, "no soft image rendered yet");
+    CU(cudaMemcpyAsync(soft_host, p->d_soft, (size_t)p->n * p->n, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
     return NHP_OK;
 }
 

@@ -99,6 +99,7 @@ struct nhp_planner {
     bool have_footprint = false;
     // images
     uint8_t *d_hard = nullptr, *d_soft = nullptr;
+    int32_t *d_dtg = nullptr;      // [n][n] column distances of the distance transform (distance.cu), soft planners only
     // run decomposition of E_Theta and the sparse tables of the image rows (render.cu)
     int4 *d_runs = nullptr;        // (db, da_lo, second look-up offset, level) of every run, grouped by Theta
     int32_t *d_run_off = nullptr;  // [nt + 1] first run of every Theta
@@ -154,4 +155,5 @@ int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);
 int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable
-int launch_soft_layouts(nhp_planner *p);              // softlayout.cu: S -> S_left, S_right, S_line
+int launch_soft_layouts(nhp_planner *p);
+int launch_soft_from_hard(nhp_planner *p, float k, float *dist_dev, int32_t *d2_dev);   // distance.cu: d_hard -> d_soft              // softlayout.cu: S -> S_left, S_right, S_line

@@ -106,6 +106,42 @@ def test_single_maneuver_sweeps_on_random_volumes(mods):
     p.close()
 
 
+def test_distance_transform_and_soft_image_on_the_device(mods):
+    """Steps 1-2 of PAPER.md:388-389 on the GPU (nhp_render_obstacles_dt) against the oracle: squared distances are
+    integers (the float32 distance is exact-to-rounding, tolerance 1e-5 as north_star asks), the soft image and
+    everything rendered and swept from it are bit-exact (rint is taken in float32 on both sides)."""
+    oracle, nhp = mods
+    import torch
+    cases = [scenes.random_scene(5, 5, 4, 21, soft=True), scenes.random_scene(7, 6, 9, 22, vehicle=(6, 3), n_rects=25, soft=True),
+             scenes.random_scene(6, 6, 8, 23, n_rects=0, soft=True), scenes.get_config(4)]
+    for sc in cases:
+        for k in (4.0, 0.0, 11.5):
+            d2, dist, soft = oracle.soft_from_hard(sc.hard, k)
+            p = nhp.Planner.from_scene(sc)
+            dist_g = torch.empty((sc.n, sc.n), dtype=torch.float32, device=p.device)
+            p.render_obstacles_dt(sc.hard, k, dist_g)
+            got = dist_g.cpu().numpy()
+            assert np.allclose(got, dist, rtol=1e-5, atol=1e-5), sc.name
+            assert (got == dist).all(), sc.name                      # in fact bit-equal: sqrt of the same integer, rounded once
+            assert (p.soft_image_numpy() == soft).all(), (sc.name, k)
+            if sc.n <= 128 and k == 4.0:
+                o, fp = oracle_for(oracle, sc)
+                Cv, Sv = o.render(fp, sc.hard, soft, method="brute")
+                assert (p.collision_numpy() == Cv).all() and (p.soft_numpy() == Sv).all(), sc.name
+                p.run_nturn(sc.start, 2)
+                assert (p.cost_volume_numpy() == o.run(Cv, Sv, sc.start, 2)).all(), sc.name
+            p.close()
+            if sc.n > 128:
+                break
+    # a planner without a soft volume refuses
+    sc = scenes.random_scene(5, 5, 4, 1)
+    p = nhp.Planner.from_scene(sc)
+    with pytest.raises(nhp.NhpError) as e:
+        p.render_obstacles_dt(sc.hard, 4.0)
+    assert e.value.code == -1
+    p.close()
+
+
 def test_errors_and_degenerate_cases(mods):
     oracle, nhp = mods
     sc = scenes.random_scene(5, 5, 4, 1)
