@@ -247,6 +247,23 @@ class Oracle:
             raise OracleError(rc, "backtrack")
         return [(w.i, w.j, w.theta, w.m) for w in out[:cnt.value]], cost.value
 
+    def goal_search(self, V, goals, d, W, w):
+        """Section IX under reading DESIGN R20: best vertex of the goal sets of `goals`
+        (list of (i, j, theta)) by V + W (di^2 + dj^2) + w dt^2.  Returns ((i, j, theta), goal index, score)."""
+        L = _load()
+        L.orc_goal_search.restype = C.c_int
+        L.orc_goal_search.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_uint32, C.c_uint32,
+                                      C.c_void_p, C.POINTER(C.c_uint64)]
+        g = np.ascontiguousarray(np.asarray(goals, np.int32).reshape(-1, 3))
+        out = np.zeros(4, np.int32)
+        score = C.c_uint64(0)
+        assert V.dtype == np.uint32 and V.flags.c_contiguous and V.shape == self.shape
+        rc = L.orc_goal_search(self._h, _ptr(V), g.ctypes.data_as(C.c_void_p), len(g), int(d), int(W), int(w),
+                               out.ctypes.data_as(C.c_void_p), C.byref(score))
+        if rc:
+            raise OracleError(rc, "goal_search")
+        return (int(out[0]), int(out[1]), int(out[2])), int(out[3]), int(score.value)
+
 
 def soft_from_hard(hard: np.ndarray, k: float = 4.0):
     """Steps 1-2 of PAPER.md:388-389 under reading DESIGN R17: exact squared distance transform of hard | wall,

@@ -695,3 +695,37 @@ int orc_soft_from_hard(const uint8_t *hard, int n, float k, int32_t *d2_out, flo
     free(g);
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Goal search, step 6 of the pipeline (section IX l.372-374): "more than one configuration
+ * in the goal set and ... a reward function (such as a function of difference to the ideal pose) over them.
+ * The optimization criterion is the reward for the vertex minus the cost to get there ... Multiple ideal
+ * goals is also possible".  Appendix G (l.1169) names the parameters: d "radius in number of grid cells",
+ * W, w "weights for goal search".  Reading DESIGN R20 (the paper gives no formula):
+ *   goal set of an ideal goal (gi, gj, gt) = vertices (gi+di, gj+dj, (gt+dt) mod N_theta) with di^2 + dj^2 <= d^2,
+ *   |dt| <= d, inside the grid (no spatial wrap), not blocked and reached (V != INF);
+ *   reward = -(W (di^2 + dj^2) + w dt^2) in cost units, so the criterion is  min  V + W (di^2 + dj^2) + w dt^2;
+ *   ties: first in the order (goal index, dt, dj, di), each ascending.
+ * Returns 0 and fills out[0..2] = (i, j, theta), out[3] = index of the ideal goal, *score; -5 if the set is empty.
+ * ------------------------------------------------------------------------------------------------ */
+int orc_goal_search(const orc_ctx *c, const uint32_t *V, const int32_t *goals, int n_goals, int d, uint32_t W, uint32_t w,
+                    int32_t *out, uint64_t *score)
+{
+    const int n = c->n, nt = c->nt;
+    uint64_t best = UINT64_MAX;
+    for (int g = 0; g < n_goals; g++)
+        for (int dt = -d; dt <= d; dt++)
+            for (int dj = -d; dj <= d; dj++)
+                for (int di = -d; di <= d; di++) {
+                    if (di * di + dj * dj > d * d) continue;
+                    const int i = goals[3 * g] + di, j = goals[3 * g + 1] + dj, t = (goals[3 * g + 2] + dt + 4 * nt) % nt;
+                    if (i < 0 || i >= n || j < 0 || j >= n) continue;
+                    const uint32_t v = V[((size_t)t * n + j) * n + i];
+                    if (v == ORC_INF) continue;
+                    const uint64_t s = (uint64_t)v + (uint64_t)W * (uint64_t)(di * di + dj * dj) + (uint64_t)w * (uint64_t)(dt * dt);
+                    if (s < best) { best = s; out[0] = i; out[1] = j; out[2] = t; out[3] = g; }
+                }
+    if (best == UINT64_MAX) return -5;
+    *score = best;
+    return 0;
+}
