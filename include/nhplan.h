@@ -174,6 +174,21 @@ int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out);
 int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *out_host, int cap,
                      int *count, uint32_t *cost);
 
+/* Steps 6-8 with a goal SET and a reward (section IX: "more than one configuration in the goal
+ * set and ... a reward function ... The optimization criterion is the reward for the vertex minus the cost to get
+ * there ... Multiple ideal goals is also possible"; parameters d, W, w of appendix G l.1169).  Reading DESIGN R20:
+ *   goal set of ideal goal g = vertices (gi+di, gj+dj, (gtheta+dt) mod N_theta), di^2 + dj^2 <= d^2, |dt| <= d,
+ *   clipped at the grid border, not blocked, reached;   criterion  min  V + W (di^2 + dj^2) + w dt^2  (cost units);
+ *   ties: first in the order (goal index, dt, dj, di), each ascending.
+ *   goals_host  HOST array of n_goals x 3 int32 (i, j, theta), 1 <= n_goals <= 256;  0 <= d <= 31;  W, w < 2^20
+ *   chosen      HOST int32[4] or NULL: the winning vertex (i, j, theta) and the index of its ideal goal
+ *   score       HOST or NULL: the criterion of the winner
+ * The search runs on the device ("to avoid transferring the value volume", l.374) and hands its result to the
+ * back-tracking kernel without a host round trip; the plan starts at the chosen vertex.  d = 0 with one goal is
+ * nhp_extract_path.  Errors as nhp_extract_path; NHP_E_GOAL_UNREACHED if no vertex of any goal set is reached. */
+int nhp_extract_path_goalset(nhp_planner *p, const int32_t *goals_host, int n_goals, int d, uint32_t W, uint32_t w,
+                             nhp_waypoint *out_host, int cap, int *count, uint32_t *cost, int32_t *chosen, uint64_t *score);
+
 /* Synchronise and report device-side conditions of the last run (NHP_OK or NHP_E_START_BLOCKED). */
 int nhp_status(nhp_planner *p);
 

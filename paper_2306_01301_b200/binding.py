@@ -18,7 +18,7 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
            "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
            "nhp_run_nturn", "nhp_run_more",
-           "nhp_cost_volume", "nhp_extract_path", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
+           "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
 KERNEL_SLOTS = 13
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
@@ -77,6 +77,8 @@ def load_library():
         L.nhp_cost_volume.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.nhp_extract_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Waypoint), C.c_int,
                                        C.POINTER(C.c_int), C.POINTER(C.c_uint32)]
+        L.nhp_extract_path_goalset.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_uint32, C.c_uint32, C.POINTER(Waypoint),
+                                               C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_uint32), C.c_void_p, C.POINTER(C.c_uint64)]
         L.nhp_status.argtypes = [C.c_void_p]
         L.nhp_index_to_pose.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int] + [C.POINTER(C.c_double)] * 3
         L.nhp_pose_to_index.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double] + [C.POINTER(C.c_int)] * 3
@@ -213,6 +215,19 @@ class Planner:
         self._check(self._L.nhp_extract_path(self._h, int(goal[0]), int(goal[1]), int(goal[2]), buf, cap,
                                              C.byref(cnt), C.byref(cost)), "extract_path")
         return [(w.i, w.j, w.theta, w.m) for w in buf[:cnt.value]], cost.value
+
+    def extract_path_goalset(self, goals, d, W, w, cap=4096):
+        """Goal search over the goal sets of `goals` (list of (i, j, theta)) + back-tracking from the winner.
+        Returns (plan, cost, (i, j, theta), goal index, score)."""
+        g = np.ascontiguousarray(np.asarray(goals, np.int32).reshape(-1, 3))
+        buf = (Waypoint * cap)()
+        cnt, cost, score = C.c_int(0), C.c_uint32(0), C.c_uint64(0)
+        chosen = np.zeros(4, np.int32)
+        self._check(self._L.nhp_extract_path_goalset(self._h, g.ctypes.data, len(g), int(d), int(W), int(w), buf, cap,
+                                                     C.byref(cnt), C.byref(cost), chosen.ctypes.data, C.byref(score)),
+                    "extract_path_goalset")
+        return ([(x.i, x.j, x.theta, x.m) for x in buf[:cnt.value]], cost.value,
+                (int(chosen[0]), int(chosen[1]), int(chosen[2])), int(chosen[3]), int(score.value))
 
     def status(self):
         self._check(self._L.nhp_status(self._h), "status")

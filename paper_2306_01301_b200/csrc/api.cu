@@ -162,11 +162,12 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     alloc((void **)&p->d_hard, npx);
     alloc((void **)&p->d_soft, npx);
     if (w->flags & NHP_FLAG_SOFT) alloc((void **)&p->d_dtg, sizeof(int32_t) * npx);
-    alloc((void **)&p->d_status, sizeof(int32_t) * 8);
+    alloc((void **)&p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS);
+    alloc((void **)&p->d_goals, sizeof(int32_t) * 3 * NHP_MAX_GOALS);
     alloc((void **)&p->d_plan, sizeof(nhp_waypoint) * p->plan_cap);
-    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * 8) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * NHP_STATUS_WORDS) != cudaSuccess) rc = NHP_E_CUDA;
     if (rc == NHP_OK && cudaMallocHost((void **)&p->h_plan, sizeof(nhp_waypoint) * p->plan_cap) != cudaSuccess) rc = NHP_E_CUDA;
-    if (rc == NHP_OK && cudaMemsetAsync(p->d_status, 0, sizeof(int32_t) * 8, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK && cudaMemsetAsync(p->d_status, 0, sizeof(int32_t) * NHP_STATUS_WORDS, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
     if (rc != NHP_OK) { nhp_planner_destroy(p); return rc; }
     *out = p;
     return NHP_OK;
@@ -179,7 +180,7 @@ int nhp_planner_destroy(nhp_planner *p)
     cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
     cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
     cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
-    cudaFree(p->d_status); cudaFree(p->d_plan); cudaFree(p->d_dtg);
+    cudaFree(p->d_status); cudaFree(p->d_plan); cudaFree(p->d_dtg); cudaFree(p->d_goals);
     if (p->h_status) cudaFreeHost(p->h_status);
     if (p->h_plan) cudaFreeHost(p->h_plan);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
@@ -299,7 +300,7 @@ int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out)
 int nhp_status(nhp_planner *p)
 {
     if (!p) return NHP_E_ARG;
-    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     if (p->have_run && p->h_status[0]) return fail(p, NHP_E_START_BLOCKED, "the start vertex collides");
     return NHP_OK;
@@ -314,7 +315,7 @@ int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *o
     if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
     p->launches += launch_backtrack(p, gi, gj, gtheta);
     CU(cudaGetLastError());
-    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * 8, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));                                             // step 8
     const int rc = p->h_status[1];
@@ -326,6 +327,39 @@ int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *o
     std::memcpy(out_host, p->h_plan, sizeof(nhp_waypoint) * n);
     *count = n;
     *cost = (uint32_t)p->h_status[3];
+    return NHP_OK;
+}
+
+int nhp_extract_path_goalset(nhp_planner *p, const int32_t *goals_host, int n_goals, int d, uint32_t W, uint32_t w,
+                             nhp_waypoint *out_host, int cap, int *count, uint32_t *cost, int32_t *chosen, uint64_t *score)
+{
+    if (!p || !goals_host || !out_host || !count || !cost || cap < 1) return fail(p, NHP_E_ARG, "bad extract_path_goalset argument");
+    if (n_goals < 1 || n_goals > NHP_MAX_GOALS || d < 0 || d > 31 || W >= (1u << 20) || w >= (1u << 20))
+        return fail(p, NHP_E_ARG, "goal set outside the supported range (<= 256 goals, d <= 31, W, w < 2^20)");
+    if ((long long)n_goals * (2 * d + 1) * (2 * d + 1) * (2 * d + 1) >= (1ll << 24)) return fail(p, NHP_E_ARG, "goal set too large");
+    if (!p->have_run) return fail(p, NHP_E_STATE, "extract_path before run_nturn");
+    for (int g = 0; g < n_goals; g++)
+        if (!in_grid(p, goals_host[3 * g], goals_host[3 * g + 1], goals_host[3 * g + 2])) return fail(p, NHP_E_ARG, "goal pose outside the grid");
+    *count = 0; *cost = NHP_INF;
+    if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
+    CU(cudaMemcpyAsync(p->d_goals, goals_host, sizeof(int32_t) * 3 * n_goals, cudaMemcpyHostToDevice, p->stream));
+    p->launches += launch_goal_search(p, n_goals, d, W, w);                           // step 6
+    p->launches += launch_backtrack(p, -1, -1, -1);                                   // step 7
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));                                             // step 8
+    const int rc = p->h_status[1];
+    if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
+    if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "no vertex of the goal set is reached");
+    if (rc != NHP_OK) return fail(p, rc, "plan longer than the internal buffer");
+    const int n = p->h_status[2];
+    if (n > cap) return fail(p, NHP_E_BUFFER, "plan longer than the caller's buffer");
+    std::memcpy(out_host, p->h_plan, sizeof(nhp_waypoint) * n);
+    *count = n;
+    *cost = (uint32_t)p->h_status[3];
+    if (chosen) for (int k = 0; k < 4; k++) chosen[k] = p->h_status[4 + k];
+    if (score) *score = (uint64_t)(uint32_t)p->h_status[8] | ((uint64_t)(uint32_t)p->h_status[9] << 32);
     return NHP_OK;
 }
 

@@ -13,6 +13,7 @@ struct BtParams {
     int log2_n, nt, fwd_only, soft;
     int si, sj, st, gi, gj, gt;
     int cap;
+    int goal_from_status;   // the goal vertex comes from goal_search_kernel (status[4..6], found flag status[10])
 };
 
 __device__ __forceinline__ unsigned long long warp_min_u64(unsigned long long x)
@@ -40,8 +41,10 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
     unsigned long long total = 0;
     if (threadIdx.x == 0) {
         int go = 1;
+        if (P.goal_from_status) { P.gi = status[4]; P.gj = status[5]; P.gt = status[6]; }
         const size_t gidx = ((((size_t)P.gt << log2_n) + P.gj) << log2_n) + P.gi;
         if (status[0]) { status[1] = NHP_E_START_BLOCKED; go = 0; }
+        else if (P.goal_from_status && !status[10]) { status[1] = NHP_E_GOAL_UNREACHED; go = 0; }
         else if (V[gidx] == 0u) { status[1] = NHP_E_GOAL_UNREACHED; go = 0; }
         else if (P.gi == P.si && P.gj == P.sj && P.gt == P.st) {
             if (P.cap < 1) status[1] = NHP_E_BUFFER;
@@ -167,6 +170,61 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Goal search, step 6 of the pipeline (section IX l.372-374; parameters d, W, w of appendix G l.1169):
+// "more than one configuration in the goal set and ... a reward function ... over them.  The optimization criterion is
+// the reward for the vertex minus the cost to get there ... Multiple ideal goals is also possible ... done on the GPU to
+// avoid transferring the value volume".  Reading DESIGN R20: goal set = disc of radius d cells around the ideal pose
+// times |dTheta| <= d, clipped at the grid border; criterion min V + W (di^2 + dj^2) + w dTheta^2; ties to the first
+// candidate in the order (goal, dTheta, dj, di).  One block; key = (score << 24) | order, 64-bit min.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) goal_search_kernel(const uint32_t *__restrict__ V, const int32_t *__restrict__ goals, int n_goals,
+                                                         int d, uint32_t W, uint32_t w, int log2_n, int nt, int32_t *__restrict__ status)
+{
+    __shared__ unsigned long long s_min[32];
+    const int n = 1 << log2_n, side = 2 * d + 1, per_goal = side * side * side, total = n_goals * per_goal;
+    unsigned long long best = ~0ull;
+    for (int c = threadIdx.x; c < total; c += blockDim.x) {
+        const int g = c / per_goal, r = c - g * per_goal;
+        const int dt = r / (side * side) - d, dj = (r / side) % side - d, di = r % side - d;
+        if (di * di + dj * dj > d * d) continue;
+        const int i = goals[3 * g] + di, j = goals[3 * g + 1] + dj, t = (goals[3 * g + 2] + dt + 4 * nt) & (nt - 1);
+        if (i < 0 || i >= n || j < 0 || j >= n) continue;
+        const uint32_t v = V[((((size_t)t << log2_n) + j) << log2_n) + i];
+        if (v == 0u || v >= VI_INF) continue;                                  // blocked / unreached (internal encoding)
+        const unsigned long long score = (unsigned long long)(v - 1u) + (unsigned long long)W * (unsigned)(di * di + dj * dj) +
+                                         (unsigned long long)w * (unsigned)(dt * dt);
+        const unsigned long long key = (score << 24) | (unsigned)c;
+        best = key < best ? key : best;
+    }
+    best = warp_min_u64(best);
+    if ((threadIdx.x & 31) == 0) s_min[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        best = threadIdx.x < (blockDim.x >> 5) ? s_min[threadIdx.x] : ~0ull;
+        best = warp_min_u64(best);
+        if (threadIdx.x == 0) {
+            status[10] = best != ~0ull;
+            if (best != ~0ull) {
+                const int c = (int)(best & 0xffffffu), g = c / per_goal, r = c - g * per_goal;
+                status[4] = goals[3 * g] + r % side - d;
+                status[5] = goals[3 * g + 1] + (r / side) % side - d;
+                status[6] = (goals[3 * g + 2] + r / (side * side) - d + 4 * nt) & (nt - 1);
+                status[7] = g;
+                status[8] = (int32_t)((best >> 24) & 0xffffffffu);
+                status[9] = (int32_t)(best >> 56);
+            }
+        }
+    }
+}
+
+int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w)
+{
+    ProfScope prof(p, 9);
+    goal_search_kernel<<<1, 1024, 0, p->stream>>>(p->V, p->d_goals, n_goals, d, W, w, p->log2_n, p->nt, p->d_status);
+    return 1;
+}
+
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt)
 {
     BtParams P;
@@ -177,6 +235,7 @@ int launch_backtrack(nhp_planner *p, int gi, int gj, int gt)
     P.si = p->start[0]; P.sj = p->start[1]; P.st = p->start[2];
     P.gi = gi; P.gj = gj; P.gt = gt;
     P.cap = p->plan_cap;
+    P.goal_from_status = gi < 0;
     ProfScope prof(p, 9);
     backtrack_kernel<<<1, 192, 0, p->stream>>>(p->V, p->S, p->tables(), P, p->d_plan, p->d_status);
     return 1;

@@ -109,7 +109,9 @@ struct nhp_planner {
     bool have_render = false, have_run = false, canonical = false;
     int start[3] = {0, 0, 0};
     // plan extraction
-    int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost
+    int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search: i, j, theta, goal
+                                   // index, [8..9] its score, [10] found; NHP_STATUS_WORDS words
+    int32_t *d_goals = nullptr;    // [NHP_MAX_GOALS][3] ideal goals of nhp_extract_path_goalset
     nhp_waypoint *d_plan = nullptr;
     int plan_cap = 0;
     int32_t *h_status = nullptr;   // pinned
@@ -128,6 +130,8 @@ struct nhp_planner {
 };
 
 constexpr int PROF_PAIRS = 1024;
+constexpr int NHP_STATUS_WORDS = 16;
+constexpr int NHP_MAX_GOALS = 256;
 
 // Bracket one kernel launch (or one group of launches) with an event pair when profiling is on.
 struct ProfScope {
@@ -153,7 +157,8 @@ int launch_render(nhp_planner *p, bool soft);
 int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
-int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);
+int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);     // gi < 0: the goal comes from launch_goal_search
+int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w);
 int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable
 int launch_soft_layouts(nhp_planner *p);
 int launch_soft_from_hard(nhp_planner *p, float k, float *dist_dev, int32_t *d2_dev);   // distance.cu: d_hard -> d_soft              // softlayout.cu: S -> S_left, S_right, S_line

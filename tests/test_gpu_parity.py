@@ -142,6 +142,44 @@ def test_distance_transform_and_soft_image_on_the_device(mods):
     p.close()
 
 
+def test_goal_search_over_goal_sets(mods):
+    """Step 6 (section IX) on the GPU against the oracle: same winner, same score, and the plan
+    extracted from it is the oracle's plan from that vertex."""
+    oracle, nhp = mods
+    rng = np.random.default_rng(7)
+    for sc in (scenes.random_scene(6, 5, 5, 31, n_rects=8, n_cycles=4), scenes.random_scene(6, 6, 8, 32, soft=True, reverse_mult=512, n_cycles=3),
+               scenes.get_config(2)):
+        o, fp = oracle_for(oracle, sc)
+        Cv, Sv = o.render(fp, sc.hard, sc.soft, method="runs")
+        V = o.run(Cv, Sv, sc.start, sc.n_cycles)
+        p = nhp.Planner.from_scene(sc)
+        p.render_obstacles(sc.hard, sc.soft)
+        p.run_nturn(sc.start, sc.n_cycles)
+        tj, jj, ij = np.nonzero(V != INF)
+        picks = rng.integers(len(tj), size=24)
+        goals = [(int(ij[k]), int(jj[k]), int(tj[k])) for k in picks] + [tuple(sc.goal), (1, 1, 0), (sc.n - 1, sc.n - 2, sc.nt - 1)]
+        for trial, g in enumerate(goals):
+            d, W, w = int(rng.integers(0, 6)), int(rng.integers(0, 3000)), int(rng.integers(0, 3000))
+            gs = [g] if trial % 3 else [g, goals[(trial + 5) % len(goals)], goals[(trial + 11) % len(goals)]]
+            try:
+                cell, gi, score = o.goal_search(V, gs, d, W, w)
+            except oracle.OracleError as e:
+                with pytest.raises(nhp.NhpError) as ge:
+                    p.extract_path_goalset(gs, d, W, w)
+                assert ge.value.code == e.code == -5
+                continue
+            plan, cost, gcell, ggi, gscore = p.extract_path_goalset(gs, d, W, w)
+            assert (gcell, ggi, gscore) == (cell, gi, score), (sc.name, gs, d, W, w)
+            assert (plan, cost) == o.backtrack(V, Cv, Sv, sc.start, cell), (sc.name, cell)
+        # d = 0, one goal == extract_path
+        g = goals[0]
+        assert p.extract_path_goalset([g], 0, 5, 5)[:2] == p.extract_path(g)
+        with pytest.raises(nhp.NhpError) as ge:
+            p.extract_path_goalset([g], 40, 1, 1)
+        assert ge.value.code == -1
+        p.close()
+
+
 def test_errors_and_degenerate_cases(mods):
     oracle, nhp = mods
     sc = scenes.random_scene(5, 5, 4, 1)
