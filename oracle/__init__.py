@@ -229,10 +229,35 @@ class Oracle:
             raise OracleError(rc, "run")
         return V
 
-    def dijkstra(self, Cv, Sv, start, kind="star"):
+    def run_from(self, Cv, Sv, start, m0, ncycles):
+        """N-turn run with maneuver m0 in progress at the start (DESIGN R26); m0 = -1: plain run."""
         V = np.empty(self.shape, np.uint32)
         self._vols(V, Cv, Sv)
-        rc = _load().orc_dijkstra(self._h, 0 if kind == "star" else 1, _ptr(Cv), _ptr(Sv), start[0], start[1], start[2], _ptr(V))
+        L = _load()
+        L.orc_run_from.argtypes = [C.c_void_p] + [C.c_void_p] * 3 + [C.c_int] * 5
+        rc = L.orc_run_from(self._h, _ptr(V), _ptr(Cv), _ptr(Sv), start[0], start[1], start[2], int(m0), ncycles)
+        if rc:
+            raise OracleError(rc, "run_from")
+        return V
+
+    def backtrack_from(self, V, Cv, Sv, start, m0, goal, cap=4096):
+        self._vols(V, Cv, Sv)
+        out = (_Waypoint * cap)()
+        cnt, cost = C.c_int(0), C.c_uint32(0)
+        L = _load()
+        L.orc_backtrack_from.argtypes = [C.c_void_p] + [C.c_void_p] * 3 + [C.c_int] * 7 + [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        rc = L.orc_backtrack_from(self._h, _ptr(V), _ptr(Cv), _ptr(Sv), start[0], start[1], start[2], int(m0),
+                                  goal[0], goal[1], goal[2], out, cap, C.byref(cnt), C.byref(cost))
+        if rc:
+            raise OracleError(rc, "backtrack")
+        return [(w.i, w.j, w.theta, w.m) for w in out[:cnt.value]], cost.value
+
+    def dijkstra(self, Cv, Sv, start, kind="star", m0=-1):
+        V = np.empty(self.shape, np.uint32)
+        self._vols(V, Cv, Sv)
+        L = _load()
+        L.orc_dijkstra_from.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        rc = L.orc_dijkstra_from(self._h, 0 if kind == "star" else 1, _ptr(Cv), _ptr(Sv), start[0], start[1], start[2], int(m0), _ptr(V))
         if rc:
             raise OracleError(rc, "dijkstra")
         return V

@@ -517,7 +517,7 @@ static hitem hpop(heap *h)
     return top;
 }
 
-int orc_dijkstra(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S, int si, int sj, int st, uint32_t *Vout)
+int orc_dijkstra_from(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S, int si, int sj, int st, int m0, uint32_t *Vout)
 {
     int n = c->n, nt = c->nt;
     size_t nr = (size_t)n * n * nt;
@@ -532,6 +532,11 @@ int orc_dijkstra(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S,
     heap h = { 0, 0, 0 };
     D[sidx * nv] = 0;
     hpush(&h, 0, (uint64_t)sidx * nv);
+    if (m0 >= 0) {                                          /* maneuver m0 is in progress at the start: */
+        if (kind != 0 || m0 > 5) { free(D); return -1; }    /* its Star vertex is a source too, so continuing it costs no c_t */
+        D[sidx * nv + 1 + m0] = 0;
+        hpush(&h, 0, (uint64_t)sidx * nv + 1 + m0);
+    }
 #define RELAX(vid, nd) do { uint32_t nd_ = (nd); uint64_t v_ = (vid); if (nd_ < D[v_]) { D[v_] = nd_; hpush(&h, nd_, v_); } } while (0)
     while (h.n) {
         hitem it = hpop(&h);
@@ -579,9 +584,11 @@ int orc_dijkstra(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S,
  * (= V[goal] once the volume has converged, <= V[goal] before).  Returns 0, -5 goal unreached,
  * -6 buffer too small.
  * ---------------------------------------------------------------------------------------- */
-int orc_backtrack(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const uint8_t *S,
-                  int si, int sj, int st, int gi, int gj, int gt,
-                  orc_waypoint *out, int cap, int *count, uint32_t *cost)
+/* m0 >= 0: maneuver m0 was in progress at the start (orc_run_from): the segment that leaves the START under m0
+ * carries no transition cost */
+int orc_backtrack_from(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const uint8_t *S,
+                       int si, int sj, int st, int m0, int gi, int gj, int gt,
+                       orc_waypoint *out, int cap, int *count, uint32_t *cost)
 {
     int n = c->n, nt = c->nt, cnt = 0;
     int fwd_only = c->p.flags & ORC_FLAG_FORWARD_ONLY;
@@ -609,8 +616,9 @@ int orc_backtrack(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const u
                 size_t q = ((size_t)qt * n + qj) * n + qi;
                 if (C[q]) break;
                 E = cadd(E, edge_w(c, S, m, qt, q));
-                uint32_t cand = cadd(cadd(V[q], c->p.ct[m]), E);
-                if (cand < best) { best = cand; bseg = cadd(c->p.ct[m], E); bi = qi; bj = qj; bt = qt; bm = m; }
+                uint32_t ctm = (m == m0 && qi == si && qj == sj && qt == st) ? 0 : c->p.ct[m];
+                uint32_t cand = cadd(cadd(V[q], ctm), E);
+                if (cand < best) { best = cand; bseg = cadd(ctm, E); bi = qi; bj = qj; bt = qt; bm = m; }
                 pi = qi; pj = qj; pt = qt;
             }
         }
@@ -624,6 +632,51 @@ int orc_backtrack(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const u
     if (cnt >= cap) return -6;
     out[cnt].i = ci; out[cnt].j = cj; out[cnt].theta = cth; out[cnt].m = -1; cnt++;
     *count = cnt; *cost = total;
+    return 0;
+}
+
+int orc_backtrack(const orc_ctx *c, const uint32_t *V, const uint8_t *C, const uint8_t *S,
+                  int si, int sj, int st, int gi, int gj, int gt,
+                  orc_waypoint *out, int cap, int *count, uint32_t *cost)
+{
+    return orc_backtrack_from(c, V, C, S, si, sj, st, -1, gi, gj, gt, out, cap, count, cost);
+}
+
+int orc_dijkstra(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S, int si, int sj, int st, uint32_t *Vout)
+{
+    return orc_dijkstra_from(c, kind, C, S, si, sj, st, -1, Vout);
+}
+
+/* Start state with a maneuver in progress (section XII: "if a maneuver is in progress, there should be
+ * no transition cost to start with that maneuver, which is easily accomplished by using the appropriate start
+ * configuration").  Reading DESIGN R26: besides V[start] = 0 the vertices AHEAD of the start on the curve of m0 are
+ * seeded with the summed edge weights from the start (no c_t), up to the first blocked vertex (at most one lap);
+ * then the cycles run as usual.  The walk uses the edge maps (25)-(31), not the sweep code. */
+int orc_run_from(const orc_ctx *c, uint32_t *V, const uint8_t *C, const uint8_t *S, int si, int sj, int st, int m0, int ncycles)
+{
+    int n = c->n, nt = c->nt;
+    size_t nr = (size_t)n * n * nt;
+    size_t sidx = ((size_t)st * n + sj) * n + si;
+    if (si < 0 || sj < 0 || st < 0 || si >= n || sj >= n || st >= nt || m0 < -1 || m0 > 5) return -1;
+    if (m0 >= 0 && (c->p.flags & ORC_FLAG_FORWARD_ONLY) && (m0 == M_RB || m0 == M_SB || m0 == M_LB)) return -1;
+    if (C[sidx]) return -4;
+    for (size_t x = 0; x < nr; x++) V[x] = ORC_INF;
+    V[sidx] = 0;
+    if (m0 >= 0) {
+        int i = si, j = sj, t = st, steps = (m0 == M_SF || m0 == M_SB) ? n : nt - 1;
+        uint32_t acc = 0;
+        for (int k = 0; k < steps; k++) {
+            int i2, j2, t2;
+            size_t X = ((size_t)t * n + j) * n + i;
+            orc_edge(c, m0, i, j, t, &i2, &j2, &t2);
+            size_t X2 = ((size_t)t2 * n + j2) * n + i2;
+            if (C[X2]) break;
+            acc = cadd(acc, edge_w(c, S, m0, t, X));
+            if (acc < V[X2]) V[X2] = acc;
+            i = i2; j = j2; t = t2;
+        }
+    }
+    orc_cycles(c, V, C, S, ncycles);
     return 0;
 }
 
