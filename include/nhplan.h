@@ -156,6 +156,15 @@ int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host);
  * Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_CUDA. */
 int nhp_run_nturn(nhp_planner *p, int i, int j, int theta, int n_cycles);
 
+/* nhp_run_nturn with a maneuver IN PROGRESS at the start (section XII: "the current maneuver state
+ * should also be encoded in the graph when a plan is in progress ... if a maneuver is in progress, there should be no
+ * transition cost to start with that maneuver").  Reading DESIGN R26: besides V[start] = 0, the vertices ahead of the
+ * start on the curve of maneuver m0 are seeded with the summed edge weights from the start, without ct[m0], up to the
+ * first blocked vertex (at most one lap); nhp_extract_path then charges no ct for the segment that leaves the start
+ * under m0.  m0 = -1: no maneuver in progress (= nhp_run_nturn).  Errors as nhp_run_nturn; NHP_E_ARG for a reverse
+ * maneuver with NHP_FLAG_FORWARD_ONLY. */
+int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cycles);
+
 /* Continue sweeping the existing value volume for n_cycles more cycles. */
 int nhp_run_more(nhp_planner *p, int n_cycles);
 

@@ -17,7 +17,7 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
 
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
            "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
-           "nhp_run_nturn", "nhp_run_more",
+           "nhp_run_nturn", "nhp_run_nturn_from", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
 KERNEL_SLOTS = 13
@@ -73,6 +73,7 @@ def load_library():
         L.nhp_render_obstacles_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
         L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
         L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.nhp_run_nturn_from.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
         L.nhp_run_more.argtypes = [C.c_void_p, C.c_int]
         L.nhp_cost_volume.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.nhp_extract_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Waypoint), C.c_int,
@@ -198,6 +199,11 @@ class Planner:
 
     def run_nturn(self, start, n_cycles=8):
         self._check(self._L.nhp_run_nturn(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_cycles)), "run_nturn")
+
+    def run_nturn_from(self, start, m0, n_cycles=8):
+        """run_nturn with maneuver m0 (0..5 in cycle order, -1 = none) in progress at the start."""
+        self._check(self._L.nhp_run_nturn_from(self._h, int(start[0]), int(start[1]), int(start[2]), int(m0), int(n_cycles)),
+                    "run_nturn_from")
 
     def run_more(self, n_cycles):
         self._check(self._L.nhp_run_more(self._h, int(n_cycles)), "run_more")

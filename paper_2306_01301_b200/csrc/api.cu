@@ -263,13 +263,23 @@ int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host)
 
 int nhp_run_nturn(nhp_planner *p, int i, int j, int theta, int n_cycles)
 {
+    return nhp_run_nturn_from(p, i, j, theta, -1, n_cycles);
+}
+
+int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cycles)
+{
     if (!p) return NHP_E_ARG;
+    if (m0 < -1 || m0 > 5) return fail(p, NHP_E_ARG, "maneuver id outside [-1, 5]");
+    if (m0 >= 0 && (p->w.flags & NHP_FLAG_FORWARD_ONLY) && (m0 == M_RB || m0 == M_SB || m0 == M_LB))
+        return fail(p, NHP_E_ARG, "a reverse maneuver cannot be in progress with NHP_FLAG_FORWARD_ONLY");
     if (!p->have_render) return fail(p, NHP_E_STATE, "run_nturn before render_obstacles");
     if (!in_grid(p, i, j, theta)) return fail(p, NHP_E_ARG, "start pose outside the grid");
     if (n_cycles <= 0) n_cycles = 8;
     p->start[0] = i; p->start[1] = j; p->start[2] = theta;
+    p->start_m0 = m0;
     p->launches += launch_init_volume(p, i, j, theta);
     p->canonical = false;
+    if (m0 >= 0) p->launches += launch_seed_in_progress(p, m0);
     p->launches += launch_cycles(p, n_cycles);
     CU(cudaGetLastError());
     p->have_run = true;

@@ -13,6 +13,7 @@ struct BtParams {
     int log2_n, nt, fwd_only, soft;
     int si, sj, st, gi, gj, gt;
     int cap;
+    int m0;                 // maneuver in progress at the start (-1: none): its segment out of the START carries no c_t
     int goal_from_status;   // the goal vertex comes from goal_search_kernel (status[4..6], found flag status[10])
 };
 
@@ -96,6 +97,7 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
             constexpr int NB = 8;                              // chunks of 32 vertices whose loads are in flight together
             for (int base = 0; base < maxk && !done; base += 32 * NB) {
                 uint32_t uu[NB], ww[NB];
+                bool at_start[NB];
 #pragma unroll
                 for (int c = 0; c < NB; c++) {
                     const int k = base + 32 * c + lane + 1;
@@ -104,6 +106,7 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
                     const size_t idx = ((((size_t)t << log2_n) + j) << log2_n) + i;
                     const bool valid = k <= maxk;
                     uu[c] = valid ? V[idx] : 0u;
+                    at_start[c] = (i == P.si && j == P.sj && t == P.st);
                     uint32_t w = T.len_q[(size_t)m * nt + t];
                     if (P.soft) w = (w * (uint32_t)(valid ? S[idx] : 16)) >> 4;
                     ww[c] = w;
@@ -125,8 +128,10 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
                     unsigned long long key = KINF;
                     uint32_t seg = 0;
                     if (lane < first && u < VI_INF) {
-                        const unsigned long long cand = (unsigned long long)(u - 1u) + ct + pre;
-                        if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ct + pre); }
+                        // u == 1 (cost 0) only at the start vertex: the maneuver in progress there is entered for free
+                        const uint32_t ctm = (m == P.m0 && u == 1u && at_start[c]) ? 0u : ct;
+                        const unsigned long long cand = (unsigned long long)(u - 1u) + ctm + pre;
+                        if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ctm + pre); }
                     }
                     const unsigned long long kmin = warp_min_u64(key);
                     if (kmin < best) {                               // strictly smaller: earlier chunks win ties
@@ -218,6 +223,79 @@ __global__ void __launch_bounds__(1024) goal_search_kernel(const uint32_t *__res
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Start state with a maneuver in progress (section XII: "if a maneuver is in progress, there should be no
+// transition cost to start with that maneuver, which is easily accomplished by using the appropriate start
+// configuration"; DESIGN R26): the vertices AHEAD of the start on the curve of m0 are seeded with the summed edge weights
+// from the start (no c_t) up to the first blocked vertex, at most one lap.  One warp, 32 vertices per step, warp prefix
+// sum; runs once per plan between the init kernel and the first sweep.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) seed_in_progress_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ S, DevTables T,
+                                                              int log2_n, int nt, int soft, int si, int sj, int st, int m)
+{
+    const int lane = threadIdx.x, n = 1 << log2_n, mx = n - 1, mt = nt - 1, quarter = nt >> 2;
+    const bool turn = !(m == M_SF || m == M_SB);
+    int xp, yp, qa = 0, qb = 0, up;
+    const int16_t *Bt = T.B + (size_t)st * n;
+    const int I = T.IJ[st] & 1, jpos = (T.IJ[st] >> 1) & 1;
+    if (turn) {
+        const bool left = (m == M_LF || m == M_LB);
+        qa = left ? 0 : 2; qb = left ? 3 : 1;
+        xp = (si - T.beta[(st + qa * quarter) & mt]) & mx;
+        yp = (sj - T.beta[(st + qb * quarter) & mt]) & mx;
+        up = (m == M_LF || m == M_RB);
+    } else {
+        yp = I ? sj : si;
+        xp = ((I ? si : sj) - Bt[yp]) & mx;
+        up = ((m == M_SF) == (jpos == 1));
+    }
+    auto cell = [&](int k, int &i, int &j, int &t) {           // vertex k steps AHEAD of the start, in the direction of m
+        if (turn) {
+            t = (up ? st + k : st - k) & mt;
+            i = (xp + T.beta[(t + qa * quarter) & mt]) & mx;
+            j = (yp + T.beta[(t + qb * quarter) & mt]) & mx;
+        } else {
+            const int y = (up ? yp + k : yp - k) & mx;
+            const int c = (xp + Bt[y]) & mx;
+            t = st; i = I ? c : y; j = I ? y : c;
+        }
+    };
+    if (V[((((size_t)st << log2_n) + sj) << log2_n) + si] == 0u) return;       // blocked start: reported by the init kernel
+    const int maxk = turn ? nt - 1 : n;
+    unsigned long long E = 0;
+    for (int base = 0; base < maxk; base += 32) {
+        const int k = base + lane + 1;
+        int i, j, t, pi, pj, pt;
+        cell(k, i, j, t);
+        cell(k - 1, pi, pj, pt);                               // the edge into vertex k is charged at its source, vertex k - 1
+        const size_t idx = ((((size_t)t << log2_n) + j) << log2_n) + i, pidx = ((((size_t)pt << log2_n) + pj) << log2_n) + pi;
+        const bool valid = k <= maxk;
+        const uint32_t u = valid ? V[idx] : 0u;
+        const unsigned blk = __ballot_sync(0xffffffffu, u == 0u);
+        const int first = blk ? __ffs(blk) - 1 : 32;
+        uint32_t w = T.len_q[(size_t)m * nt + pt];
+        if (soft) w = (w * (uint32_t)S[pidx]) >> 4;
+        unsigned long long pre = (lane < first) ? w : 0;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned long long y = __shfl_up_sync(0xffffffffu, pre, d);
+            if (lane >= d) pre += y;
+        }
+        pre += E;
+        if (lane < first && pre < NHP_COST_LIMIT && (uint32_t)pre + 1u < u) V[idx] = (uint32_t)pre + 1u;
+        E = __shfl_sync(0xffffffffu, pre, 31);
+        if (first < 32) break;
+    }
+}
+
+int launch_seed_in_progress(nhp_planner *p, int m0)
+{
+    ProfScope prof(p, 8);
+    const int soft = (p->S != nullptr && (p->w.flags & NHP_FLAG_SOFT)) ? 1 : 0;
+    seed_in_progress_kernel<<<1, 32, 0, p->stream>>>(p->V, p->S, p->tables(), p->log2_n, p->nt, soft, p->start[0], p->start[1], p->start[2], m0);
+    return 1;
+}
+
 int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w)
 {
     ProfScope prof(p, 9);
@@ -236,6 +314,7 @@ int launch_backtrack(nhp_planner *p, int gi, int gj, int gt)
     P.gi = gi; P.gj = gj; P.gt = gt;
     P.cap = p->plan_cap;
     P.goal_from_status = gi < 0;
+    P.m0 = p->start_m0;
     ProfScope prof(p, 9);
     backtrack_kernel<<<1, 192, 0, p->stream>>>(p->V, p->S, p->tables(), P, p->d_plan, p->d_status);
     return 1;

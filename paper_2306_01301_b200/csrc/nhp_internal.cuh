@@ -108,6 +108,7 @@ struct nhp_planner {
     uint8_t *d_Mk = nullptr;       // [levels][n][n]    soft image; level k = max over 2^k columns (soft only)
     bool have_render = false, have_run = false, canonical = false;
     int start[3] = {0, 0, 0};
+    int start_m0 = -1;             // maneuver in progress at the start (nhp_run_nturn_from), -1 = none
     // plan extraction
     int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search: i, j, theta, goal
                                    // index, [8..9] its score, [10] found; NHP_STATUS_WORDS words
@@ -159,6 +160,7 @@ int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);     // gi < 0: the goal comes from launch_goal_search
 int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w);
+int launch_seed_in_progress(nhp_planner *p, int m0);
 int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable
 int launch_soft_layouts(nhp_planner *p);
 int launch_soft_from_hard(nhp_planner *p, float k, float *dist_dev, int32_t *d2_dev);   // distance.cu: d_hard -> d_soft              // softlayout.cu: S -> S_left, S_right, S_line

@@ -142,6 +142,36 @@ def test_distance_transform_and_soft_image_on_the_device(mods):
     p.close()
 
 
+def test_start_state_with_a_maneuver_in_progress(mods):
+    """Section XII: no transition cost for the maneuver in progress at the start; volumes and plans
+    against the oracle for every maneuver id."""
+    oracle, nhp = mods
+    rng = np.random.default_rng(9)
+    for sc in (scenes.random_scene(5, 5, 4, 41, n_rects=5, n_cycles=3, soft=True, reverse_mult=384),
+               scenes.random_scene(7, 6, 9, 42, vehicle=(6, 3), n_rects=20, n_cycles=2), scenes.random_scene(6, 6, 8, 43, flags=1, n_cycles=2)):
+        o, fp = oracle_for(oracle, sc)
+        Cv, Sv = o.render(fp, sc.hard, sc.soft, method="runs")
+        p = nhp.Planner.from_scene(sc)
+        p.render_obstacles(sc.hard, sc.soft)
+        for m0 in range(-1, 6):
+            if (sc.flags & 1) and m0 in (2, 4, 5):
+                with pytest.raises(nhp.NhpError) as e:
+                    p.run_nturn_from(sc.start, m0, sc.n_cycles)
+                assert e.value.code == -1
+                continue
+            V = o.run_from(Cv, Sv, sc.start, m0, sc.n_cycles)
+            p.run_nturn_from(sc.start, m0, sc.n_cycles)
+            got = p.cost_volume_numpy()
+            assert (got == V).all(), (sc.name, m0, int((got != V).sum()))
+            tj, jj, ij = np.nonzero(V != INF)
+            for k in rng.integers(len(tj), size=15):
+                goal = (int(ij[k]), int(jj[k]), int(tj[k]))
+                assert p.extract_path(goal) == o.backtrack_from(V, Cv, Sv, sc.start, m0, goal), (sc.name, m0, goal)
+        p.run_nturn(sc.start, 1)                                  # a plain run afterwards forgets the maneuver
+        assert (p.cost_volume_numpy() == o.run(Cv, Sv, sc.start, 1)).all()
+        p.close()
+
+
 def test_goal_search_over_goal_sets(mods):
     """Step 6 (section IX) on the GPU against the oracle: same winner, same score, and the plan
     extracted from it is the oracle's plan from that vertex."""
