@@ -188,34 +188,58 @@ __global__ void __launch_bounds__(256) render_collision_kernel(uint32_t *__restr
 }
 
 // ---------------------------------------------------------------------------------------------
-// Soft volume: S = clamp(max over E_Theta of soft, 16, 255) (DESIGN R16), four poses per thread.
+// Soft volume: S = clamp(max over E_Theta of soft, 16, 255) (DESIGN R16), sixteen poses per thread.
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t window4(const uint32_t *__restrict__ row, int a, int mq)
+// 16 consecutive bytes of an image row starting at byte `a` (toroidal), as four words: two aligned 16-byte loads cover
+// the window, WS = (a & 15) >> 2 (the same for every thread of a run, so the caller branches on it uniformly)
+template <int WS>
+__device__ __forceinline__ uint4 window16(const uint4 *__restrict__ row, int a, int mQ)
 {
-    const int q0 = (a >> 2) & mq;
-    return __funnelshift_r(__ldg(row + q0), __ldg(row + ((q0 + 1) & mq)), (a & 3) * 8);
+    const int Q0 = (a >> 4) & mQ;
+    const uint4 lo = __ldg(row + Q0), hi = __ldg(row + ((Q0 + 1) & mQ));
+    const uint32_t w[8] = {lo.x, lo.y, lo.z, lo.w, hi.x, hi.y, hi.z, hi.w};
+    const int bs = (a & 3) * 8;
+    return make_uint4(__funnelshift_r(w[WS], w[WS + 1], bs), __funnelshift_r(w[WS + 1], w[WS + 2], bs),
+                      __funnelshift_r(w[WS + 2], w[WS + 3], bs), __funnelshift_r(w[WS + 3], w[WS + 4], bs));
 }
 
-__global__ void __launch_bounds__(256) render_soft_kernel(uint32_t *__restrict__ S4, const uint32_t *__restrict__ Mk,
+template <int WS>
+__device__ __forceinline__ void soft_run(uint4 &acc, const uint4 *__restrict__ row, int a, int mQ)
+{
+    const uint4 x = window16<WS>(row, a, mQ);
+    acc.x = __vmaxu4(acc.x, x.x); acc.y = __vmaxu4(acc.y, x.y); acc.z = __vmaxu4(acc.z, x.z); acc.w = __vmaxu4(acc.w, x.w);
+}
+
+// Sixteen poses per thread: per run two look-ups of 16 bytes each (four aligned 16-byte loads) instead of sixteen 4-byte
+// loads, and a quarter of the per-run bookkeeping per pose.
+__global__ void __launch_bounds__(256) render_soft_kernel(uint4 *__restrict__ S16, const uint4 *__restrict__ Mk,
                                                          const int4 *__restrict__ runs, const int32_t *__restrict__ run_off, int n)
 {
     extern __shared__ int4 srun[];
-    const int nq = n >> 2, mx = n - 1, mq = nq - 1;
+    const int nQ = n >> 4, mx = n - 1, mQ = nQ - 1;
     const int t = blockIdx.z;
     const int r0 = run_off[t], cnt = run_off[t + 1] - r0;
     for (int k = threadIdx.x + threadIdx.y * blockDim.x; k < cnt; k += blockDim.x * blockDim.y) srun[k] = runs[r0 + k];
     __syncthreads();
-    const int iq = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
-    if (iq >= nq) return;
-    const size_t lvl = (size_t)n * nq;
-    uint32_t acc = 0x10101010u;                                  // >= 16 = 1.0
+    const int iQ = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
+    if (iQ >= nQ) return;
+    const size_t lvl = (size_t)n * nQ;
+    uint4 acc = make_uint4(0x10101010u, 0x10101010u, 0x10101010u, 0x10101010u);   // >= 16 = 1.0
     for (int k = 0; k < cnt; k++) {
-        const int4 r = srun[k];
-        const uint32_t *row = Mk + r.w * lvl + (size_t)((j + r.x) & mx) * nq;
-        const int a = (iq << 2) + r.y;
-        acc = __vmaxu4(acc, __vmaxu4(window4(row, a, mq), window4(row, a + r.z, mq)));
+        const int4 r = srun[k];                                  // db, da_lo, second look-up offset, level
+        const uint4 *row = Mk + r.w * lvl + (size_t)((j + r.x) & mx) * nQ;
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            const int a = (iQ << 4) + r.y + (h ? r.z : 0);
+            switch ((a & 15) >> 2) {                             // uniform over the block: a = 16 iQ + (run constant)
+            case 0: soft_run<0>(acc, row, a, mQ); break;
+            case 1: soft_run<1>(acc, row, a, mQ); break;
+            case 2: soft_run<2>(acc, row, a, mQ); break;
+            default: soft_run<3>(acc, row, a, mQ); break;
+            }
+        }
     }
-    S4[((size_t)t * n + j) * nq + iq] = acc;
+    S16[((size_t)t * n + j) * nQ + iQ] = acc;
 }
 
 int launch_render(nhp_planner *p, bool soft)
@@ -241,8 +265,9 @@ int launch_render(nhp_planner *p, bool soft)
     }
     if (soft) {
         ProfScope prof(p, 7);
-        const dim3 block(nq < 32 ? nq : 32, 8);
-        render_soft_kernel<<<dim3(nq / block.x, n / 8, p->nt), block, smem, p->stream>>>((uint32_t *)p->S, (const uint32_t *)p->d_Mk,
+        const int nQ = n / 16;
+        const dim3 block(nQ < 32 ? nQ : 32, 8);
+        render_soft_kernel<<<dim3(nQ / block.x, n / 8, p->nt), block, smem, p->stream>>>((uint4 *)p->S, (const uint4 *)p->d_Mk,
                                                                                        p->d_runs, p->d_run_off, n);
         launches++;
         launches += launch_soft_layouts(p);
