@@ -234,7 +234,10 @@ struct SecLoop {
         if (GATE) { ta = nhp_gate(ta, ua); tb = nhp_gate(tb, ub); }
         wa = sec_weight<SOFT, ka>(sw, qa);
         wb = sec_weight<SOFT, kb>(sw, qb);
-        if (SOFT) { da += wa; db += wb; }
+        if (SOFT) {                                              // on the FMA pipe (IMAD with the parameter 1), not the ALU pipe
+            asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(da) : "r"(wa), "r"(one));
+            asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(db) : "r"(wb), "r"(one));
+        }
         SecLoop<L, UP, SOFT, CS, GATE, S + 1>::summary(col, sw, qa, qb, ta, wa, da, tb, wb, db, acc, one);
     }
     // apply pass: the vertex keeps min(v, u), then the same step
