@@ -203,11 +203,25 @@ __device__ __forceinline__ uint4 window16(const uint4 *__restrict__ row, int a, 
                       __funnelshift_r(w[WS + 2], w[WS + 3], bs), __funnelshift_r(w[WS + 3], w[WS + 4], bs));
 }
 
-template <int WS>
-__device__ __forceinline__ void soft_run(uint4 &acc, const uint4 *__restrict__ row, int a, int mQ)
+// Byte-wise maximum without the (emulated, ~9 instructions) __vmaxu4: the running maximum is kept as two words of
+// 16-bit lanes (even bytes, odd bytes); the two windows of a run cost four PRMT and two packed three-input 16-bit max
+// ops (VIMNMX3.S16x2; the lanes are <= 255, so the signed form is exact) per word.
+struct Max16 { uint32_t e[4], o[4]; };
+
+__device__ __forceinline__ void max16_add(Max16 &m, int k, uint32_t x, uint32_t y)
 {
-    const uint4 x = window16<WS>(row, a, mQ);
-    acc.x = __vmaxu4(acc.x, x.x); acc.y = __vmaxu4(acc.y, x.y); acc.z = __vmaxu4(acc.z, x.z); acc.w = __vmaxu4(acc.w, x.w);
+    m.e[k] = __vimax3_s16x2(m.e[k], __byte_perm(x, 0u, 0x4240), __byte_perm(y, 0u, 0x4240));     // bytes 0, 2 -> 16-bit lanes
+    m.o[k] = __vimax3_s16x2(m.o[k], __byte_perm(x, 0u, 0x4341), __byte_perm(y, 0u, 0x4341));     // bytes 1, 3
+}
+
+__device__ __forceinline__ uint4 soft_window(const uint4 *__restrict__ row, int a, int mQ)
+{
+    switch ((a & 15) >> 2) {                                     // uniform over the block: a = 16 iQ + (run constant)
+    case 0: return window16<0>(row, a, mQ);
+    case 1: return window16<1>(row, a, mQ);
+    case 2: return window16<2>(row, a, mQ);
+    default: return window16<3>(row, a, mQ);
+    }
 }
 
 // Sixteen poses per thread: per run two look-ups of 16 bytes each (four aligned 16-byte loads) instead of sixteen 4-byte
@@ -224,22 +238,18 @@ __global__ void __launch_bounds__(256) render_soft_kernel(uint4 *__restrict__ S1
     const int iQ = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y * blockDim.y + threadIdx.y;
     if (iQ >= nQ) return;
     const size_t lvl = (size_t)n * nQ;
-    uint4 acc = make_uint4(0x10101010u, 0x10101010u, 0x10101010u, 0x10101010u);   // >= 16 = 1.0
+    Max16 acc;
+#pragma unroll
+    for (int e = 0; e < 4; e++) acc.e[e] = acc.o[e] = 0x00100010u;               // >= 16 = 1.0
     for (int k = 0; k < cnt; k++) {
         const int4 r = srun[k];                                  // db, da_lo, second look-up offset, level
         const uint4 *row = Mk + r.w * lvl + (size_t)((j + r.x) & mx) * nQ;
-#pragma unroll
-        for (int h = 0; h < 2; h++) {
-            const int a = (iQ << 4) + r.y + (h ? r.z : 0);
-            switch ((a & 15) >> 2) {                             // uniform over the block: a = 16 iQ + (run constant)
-            case 0: soft_run<0>(acc, row, a, mQ); break;
-            case 1: soft_run<1>(acc, row, a, mQ); break;
-            case 2: soft_run<2>(acc, row, a, mQ); break;
-            default: soft_run<3>(acc, row, a, mQ); break;
-            }
-        }
+        const int a = (iQ << 4) + r.y;
+        const uint4 x = soft_window(row, a, mQ), y = soft_window(row, a + r.z, mQ);
+        max16_add(acc, 0, x.x, y.x); max16_add(acc, 1, x.y, y.y); max16_add(acc, 2, x.z, y.z); max16_add(acc, 3, x.w, y.w);
     }
-    S16[((size_t)t * n + j) * nQ + iQ] = acc;
+    S16[((size_t)t * n + j) * nQ + iQ] = make_uint4(acc.e[0] | (acc.o[0] << 8), acc.e[1] | (acc.o[1] << 8), acc.e[2] | (acc.o[2] << 8),
+                                                    acc.e[3] | (acc.o[3] << 8));
 }
 
 int launch_render(nhp_planner *p, bool soft)
