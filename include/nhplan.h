@@ -125,6 +125,12 @@ const char *nhp_last_error(const nhp_planner *p);
 int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int mw, int mh,
                                  double origin_u, double origin_v);
 
+/* Bounding-box vehicle as in appendix G ("f, r, s: forward, reverse and sideways bounding box dimensions
+ * in number of grid cells"): the rectangle u in [-r, f), v in [-s, s) around the centre of the rear axle, i.e.
+ * nhp_render_vehicle_footprint with the all-ones (f + r) x 2 s mask and origin (r - 1/2, s - 1/2).
+ * Errors: NHP_E_ARG, NHP_E_CUDA. */
+int nhp_set_box(nhp_planner *p, int f, int r, int s);
+
 /* Obstacle rendering, steps 3-4 of PAPER.md:390-391 (section VI l.338, appendix C l.871).
  *   hard  N x N uint8 image, row = y (j), column = x (i); non-zero = hard obstacle
  *   soft  N x N uint8 Q4.4 speed-reciprocal image (16 = 1.0) or NULL; requires NHP_FLAG_SOFT

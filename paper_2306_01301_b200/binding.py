@@ -16,7 +16,7 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
           -5: "NHP_E_GOAL_UNREACHED", -6: "NHP_E_BUFFER", -7: "NHP_E_CUDA", -8: "NHP_E_STATE", -9: "NHP_E_WEIGHTS"}
 
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
-           "nhp_render_vehicle_footprint", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
+           "nhp_render_vehicle_footprint", "nhp_set_box", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
@@ -69,6 +69,7 @@ def load_library():
         L.nhp_last_error.argtypes = [C.c_void_p]
         L.nhp_last_error.restype = C.c_char_p
         L.nhp_render_vehicle_footprint.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double]
+        L.nhp_set_box.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
         L.nhp_render_obstacles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.nhp_render_obstacles_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
         L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
@@ -158,6 +159,10 @@ class Planner:
         mask = np.ascontiguousarray(mask, np.uint8)
         self._check(self._L.nhp_render_vehicle_footprint(self._h, mask.ctypes.data, mask.shape[1], mask.shape[0],
                                                          float(origin_u), float(origin_v)), "render_vehicle_footprint")
+
+    def set_box(self, f, r, s):
+        """Bounding-box vehicle of appendix G: u in [-r, f), v in [-s, s) cells around the rear axle."""
+        self._check(self._L.nhp_set_box(self._h, int(f), int(r), int(s)), "set_box")
 
     def render_obstacles(self, hard, soft=None):
         """hard / soft: numpy uint8 arrays or CPU torch tensors (host path, copied inside the call) or CUDA tensors."""

@@ -217,6 +217,14 @@ int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int m
     return NHP_OK;
 }
 
+int nhp_set_box(nhp_planner *p, int f, int r, int s)
+{
+    if (!p || f < 0 || r < 0 || s < 1 || f + r < 1 || f + r > 1024 || 2 * s > 1024) return fail(p, NHP_E_ARG, "bad bounding box");
+    // vehicle-frame rectangle u in [-r, f), v in [-s, s): all-ones mask, pixel 0 centred at (-r + 1/2, -s + 1/2)
+    const std::vector<uint8_t> mask((size_t)(f + r) * (2 * s), 1);
+    return nhp_render_vehicle_footprint(p, mask.data(), f + r, 2 * s, (double)r - 0.5, (double)s - 0.5);
+}
+
 int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *soft, int on_device)
 {
     if (!p || !hard) return fail(p, NHP_E_ARG, "hard image is NULL");

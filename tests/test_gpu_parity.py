@@ -142,6 +142,26 @@ def test_distance_transform_and_soft_image_on_the_device(mods):
     p.close()
 
 
+def test_bounding_box_vehicle_of_appendix_g(mods):
+    """nhp_set_box(f, r, s) == the rectangle u in [-r, f), v in [-s, s): collision volume against the
+    oracle's brute-force rendering of that rectangle as a mask."""
+    oracle, nhp = mods
+    sc = scenes.random_scene(6, 6, 8, 51, n_rects=8)
+    o, _ = oracle_for(oracle, sc)
+    for f, r, s in ((5, 1, 1), (8, 2, 2), (3, 0, 1), (6, 3, 3)):
+        fp = oracle.Footprint(np.ones((2 * s, f + r), np.uint8), r - 0.5, s - 0.5)
+        Cv, _ = o.render(fp, sc.hard, None, method="brute")
+        p = nhp.Planner(sc.log2_n, sc.log2_nt, sc.R, sc.ct)
+        p.set_box(f, r, s)
+        p.render_obstacles(sc.hard)
+        assert (p.collision_numpy() == Cv).all(), (f, r, s)
+        p.close()
+    with pytest.raises(nhp.NhpError) as e:
+        p = nhp.Planner(sc.log2_n, sc.log2_nt, sc.R, sc.ct)
+        p.set_box(0, 0, 1)
+    assert e.value.code == -1
+
+
 def test_start_state_with_a_maneuver_in_progress(mods):
     """Section XII: no transition cost for the maneuver in progress at the start; volumes and plans
     against the oracle for every maneuver id."""
