@@ -272,6 +272,30 @@ class Oracle:
             raise OracleError(rc, "backtrack")
         return [(w.i, w.j, w.theta, w.m) for w in out[:cnt.value]], cost.value
 
+    def reach_run(self, Cv, start, n_levels):
+        """Appendix C: K[X] = fewest maneuvers that reach X (255 = more than n_levels), uint8."""
+        K = np.empty(self.shape, np.uint8)
+        L = _load()
+        L.orc_reach_run.restype = C.c_int
+        L.orc_reach_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+        assert Cv.dtype == np.uint8 and Cv.flags.c_contiguous and Cv.shape == self.shape
+        rc = L.orc_reach_run(self._h, _ptr(K), _ptr(Cv), start[0], start[1], start[2], int(n_levels))
+        if rc:
+            raise OracleError(rc, "reach_run")
+        return K
+
+    def reach_backtrack(self, K, Cv, start, goal, cap=4096):
+        out = (_Waypoint * cap)()
+        cnt, cost = C.c_int(0), C.c_uint32(0)
+        L = _load()
+        L.orc_reach_backtrack.restype = C.c_int
+        L.orc_reach_backtrack.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p] + [C.c_int] * 6 + [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        rc = L.orc_reach_backtrack(self._h, _ptr(K), _ptr(Cv), start[0], start[1], start[2], goal[0], goal[1], goal[2],
+                                   out, cap, C.byref(cnt), C.byref(cost))
+        if rc:
+            raise OracleError(rc, "reach_backtrack")
+        return [(w.i, w.j, w.theta, w.m) for w in out[:cnt.value]], cost.value
+
     def goal_search(self, V, goals, d, W, w):
         """Section IX under reading DESIGN R20: best vertex of the goal sets of `goals`
         (list of (i, j, theta)) by V + W (di^2 + dj^2) + w dt^2.  Returns ((i, j, theta), goal index, score)."""

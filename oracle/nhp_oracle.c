@@ -782,3 +782,103 @@ int orc_goal_search(const orc_ctx *c, const uint32_t *V, const int32_t *goals, i
     *score = best;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * Reachability ("bit-vector") planner, appendix C: edge weights zero on maneuver edges
+ * (infinite at obstacles), one on transition edges; "the value of a vertex during maneuver processing can be
+ * represented by a single bit.  That bit indicates ... if the vertex can be reached in m maneuvers or less".
+ * "The maneuver kernels now read from the previous reachability volume (at m maneuvers) ... and produce the
+ * reachability of one of the volumes of maneuver vertices (at m maneuvers plus that maneuver), which is combined
+ * ... into the reachability of the transition vertices (at m + 1 maneuvers)" -- a Jacobi step per level; the loop
+ * body is Insert 2 (l.873-878): v &= Vi[i]; Vo[i] = v; v |= B[i]  (their bit is 0 = reachable; here 1 = reachable:
+ * v |= Li[i]; blocked -> v = 0, else Lo[i] |= v).  Blocked vertices are removed (DESIGN R10).  "The output
+ * reachability bit volumes are kept around to support back-tracking" (l.897).
+ * The oracle keeps one byte per vertex: K[X] = smallest m with X reachable in <= m maneuvers, 255 = not within
+ * n_levels (n_levels <= 254).  The level volumes are L_m = (K <= m).
+ * ------------------------------------------------------------------------------------------------ */
+static void reach_sweep(const orc_ctx *c, int m, const uint8_t *K, uint8_t *Knew, const uint8_t *C, int level)
+{
+    int n = c->n, nt = c->nt;
+    int turn = !(m == M_SF || m == M_SB);
+    int n1 = turn ? n : nt, len = turn ? nt : n;
+#pragma omp parallel for num_threads(c->threads) schedule(static)
+    for (int c1 = 0; c1 < n1; c1++)
+        for (int c0 = 0; c0 < n; c0++) {
+            int steps, up;
+            if (turn) { steps = 2 * nt; up = (m == M_LF || m == M_RB); }          /* two full loops, l.356 */
+            else { steps = n; up = ((m == M_SF) == (c->J[c1] > 0)); }
+            int v = 0;
+            for (int s = 0; s < steps; s++) {
+                int k = up ? (s % len) : (len - 1 - (s % len)), i, j, t;
+                orc_curve_cell(c, m, c0, c1, k, &i, &j, &t);
+                size_t idx = ((size_t)t * n + j) * n + i;
+                if (C[idx]) { v = 0; continue; }
+                if (K[idx] <= level) v = 1;                      /* reachable at <= level maneuvers: v |= Li[i] */
+                if (v && Knew[idx] > level + 1) Knew[idx] = (uint8_t)(level + 1);
+            }
+        }
+}
+
+int orc_reach_run(const orc_ctx *c, uint8_t *K, const uint8_t *C, int si, int sj, int st, int n_levels)
+{
+    int n = c->n, nt = c->nt;
+    size_t nr = (size_t)n * n * nt, sidx = ((size_t)st * n + sj) * n + si;
+    int fwd_only = c->p.flags & ORC_FLAG_FORWARD_ONLY;
+    if (si < 0 || sj < 0 || st < 0 || si >= n || sj >= n || st >= nt || n_levels < 0 || n_levels > 254) return -1;
+    if (C[sidx]) return -4;
+    uint8_t *Kn = (uint8_t *)malloc(nr);
+    if (!Kn) return -7;
+    memset(K, 255, nr);
+    K[sidx] = 0;
+    for (int level = 0; level < n_levels; level++) {
+        memcpy(Kn, K, nr);
+        for (int m = 0; m < 6; m++) {
+            if (fwd_only && (m == M_RB || m == M_SB || m == M_LB)) continue;
+            reach_sweep(c, m, K, Kn, C, level);                  /* all six read level m, write level m + 1 */
+        }
+        memcpy(K, Kn, nr);
+    }
+    free(Kn);
+    return 0;
+}
+
+/* Back-tracking over the level volumes: from the goal at its level k, the maneuvers in cycle order; for each, walk
+ * back along its curve (against its direction) until a blocked vertex; the first vertex reachable at <= k - 1
+ * maneuvers is that maneuver's candidate; the first maneuver with a candidate wins (DESIGN R27).  Records as in
+ * orc_backtrack; *cost = number of maneuvers. */
+int orc_reach_backtrack(const orc_ctx *c, const uint8_t *K, const uint8_t *C, int si, int sj, int st, int gi, int gj, int gt,
+                        orc_waypoint *out, int cap, int *count, uint32_t *cost)
+{
+    int n = c->n, nt = c->nt, cnt = 0;
+    int fwd_only = c->p.flags & ORC_FLAG_FORWARD_ONLY;
+    int ci = gi, cj = gj, cth = gt;
+    *count = 0; *cost = ORC_INF;
+    size_t gidx = ((size_t)gt * n + gj) * n + gi;
+    if (C[gidx] || K[gidx] == 255) return -5;
+    const int total = K[gidx];
+    while (!(ci == si && cj == sj && cth == st)) {
+        int k = K[((size_t)cth * n + cj) * n + ci], found = 0, bi = 0, bj = 0, bt = 0, bm = -1;
+        if (k == 0 || k == 255) return -5;
+        for (int m = 0; m < 6 && !found; m++) {
+            if (fwd_only && (m == M_RB || m == M_SB || m == M_LB)) continue;
+            int maxk = (m == M_SF || m == M_SB) ? n : nt - 1;
+            int pi = ci, pj = cj, pt = cth;
+            for (int s = 1; s <= maxk; s++) {
+                int qi, qj, qt;
+                orc_edge(c, INV_M[m], pi, pj, pt, &qi, &qj, &qt);
+                size_t q = ((size_t)qt * n + qj) * n + qi;
+                if (C[q]) break;
+                if (K[q] <= k - 1) { found = 1; bi = qi; bj = qj; bt = qt; bm = m; break; }
+                pi = qi; pj = qj; pt = qt;
+            }
+        }
+        if (!found) return -5;
+        if (cnt >= cap) return -6;
+        out[cnt].i = ci; out[cnt].j = cj; out[cnt].theta = cth; out[cnt].m = bm; cnt++;
+        ci = bi; cj = bj; cth = bt;
+    }
+    if (cnt >= cap) return -6;
+    out[cnt].i = ci; out[cnt].j = cj; out[cnt].theta = cth; out[cnt].m = -1; cnt++;
+    *count = cnt; *cost = (uint32_t)total;
+    return 0;
+}
