@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--cycles", type=int, default=0, help="override N_T (0 = the config's own)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--simple-kernels", action="store_true", help="thread-per-curve bring-up kernels (A/B)")
+    ap.add_argument("--reach", action="store_true",
+                    help="time the reachability (bit-vector) planner of appendix C instead: render + N_T levels + back-track")
     ap.add_argument("--dt-on-device", action="store_true",
                     help="soft configs: distance transform + soft image on the GPU (nhp_render_obstacles_dt) instead of the harness image")
     return ap.parse_args()
@@ -157,6 +159,16 @@ def run_ours(args):
     dt_dev = args.dt_on_device and sc.soft is not None
 
     def step(hard, soft):
+        if args.reach:
+            p.render_obstacles(hard, None if not p.flags & 2 else soft)
+            p.reach_run(sc.start, n_cycles)
+            try:
+                state["plan"] = p.reach_extract_path(state["goal"])
+            except nhp.NhpError as e:
+                if e.code != -5:
+                    raise
+                state["plan"] = ([], 0xFFFFFFFF)
+            return
         if dt_dev:
             p.render_obstacles_dt(hard, 4.0)                       # pipeline steps 1-4 on the device
         else:
@@ -172,8 +184,15 @@ def run_ours(args):
     # warm-up, then choose a goal the sweeps actually reach (fixed for all timed steps)
     for _ in range(max(args.warmup, 1)):
         step(hard_d, soft_d)
-    p.status()
-    state["goal"] = pick_goal(p, sc, torch)
+    if args.reach:
+        K = p.reach_count_numpy()
+        cands = [tuple(sc.goal)] + [tuple(g) for g in sc.extra_goals]
+        reached = [g for g in cands if K[g[2], g[1], g[0]] != 255]
+        state["goal"] = reached[0] if K[sc.goal[2], sc.goal[1], sc.goal[0]] != 255 or not reached else max(reached, key=lambda g: K[g[2], g[1], g[0]])
+        del K
+    else:
+        p.status()
+        state["goal"] = pick_goal(p, sc, torch)
     step(hard_d, soft_d)
 
     def timed(hard, soft, profile):
@@ -211,6 +230,8 @@ def run_ours(args):
     alg_b = ALG_BYTES_SOFT if sc.soft is not None else ALG_BYTES_HARD
     # sweep kernels by slot: a single maneuver per launch (N_R pose-updates), or a turn pair (RB+RF / LB+LF: 2 N_R)
     sweeps = {k: v for k, v in kt.items() if (k in nhp.MANEUVER_NAMES or k == "turn_pair") and v[1]}
+    if args.reach:
+        return finish_reach(args, sc, n_cycles, n_r, ws, ms_dev_max, ms_e2e_max, units, launches, kt, clk, state, peak, peak_src, hard_h, p, replicas)
     dom = max(sweeps, key=lambda k: sweeps[k][0])
     dom_ms, dom_n = sweeps[dom]
     per_launch_bytes = alg_b * n_r * (2 if dom == "turn_pair" else 1)
@@ -218,7 +239,7 @@ def run_ours(args):
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
     traffic = measured_traffic(args.config, dom)
-    # secondary bound (DESIGN.md 6.6): the integer min/max pipe, 16 lanes per SM sub-partition and clock
+    # secondary bound (DESIGN.md 6.7): the integer min/max pipe, 16 lanes per SM sub-partition and clock
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     sm_clock = (clk or {}).get("sm_mhz") or 1965.0
     alu_peak = sm_count * 4 * 16 * sm_clock * 1e6 / 1e12                       # T lane-ops / s
@@ -246,12 +267,40 @@ def run_ours(args):
                      "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
         "alu": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": alu_peak, "unit": "T min/max lane-ops/s",
                 "frac": alu_achieved / alu_peak, "ops_per_pose_update": ops_per_update,
-                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.6)"},
+                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.7)"},
         "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
         "ms_per_step_with_kernel_events": ms_prof / args.steps,
     }
     if not args.no_cpu_baseline and ws == 1:
         out["cpu_baseline"] = cpu_baseline(sc, n_cycles, sample_cycles=2)
+    p.close()
+    replicas.shutdown()
+    print(json.dumps(out), flush=True)
+
+
+def finish_reach(args, sc, n_cycles, n_r, ws, ms_dev_max, ms_e2e_max, units, launches, kt, clk, state, peak, peak_src, hard_h, p, replicas):
+    """JSON line of the reachability planner (appendix C): same metric, a pose-update = one bit visited by one maneuver sweep
+    of one level; algorithmic bytes per pose-update = read the level bit + the collision bit, write the next level's bit."""
+    lv_ms, lv_n = kt.get("reach_level", (0.0, 0))
+    per_launch_bytes = 0.375 * 6 * n_r
+    achieved = per_launch_bytes / (lv_ms / max(lv_n, 1) * 1e-3) / 1e9 if lv_ms > 0 else 0.0
+    plan, nm = state["plan"]
+    out = {
+        "metric": METRIC.replace("N-turn planner", "reachability (bit-vector) planner, appendix C"), "value": units / (ms_dev_max * 1e-3) / 1e9,
+        "unit": UNIT, "n_gpus": ws, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u1 (bit per pose)", "data": "synthetic",
+        "config": {"workload": workload_name(sc, n_cycles) + ", reachability planner: N_T levels", "baseline_config": args.config,
+                   "goal": list(state["goal"]), "plan_waypoints": len(plan), "plan_maneuvers": nm,
+                   "l2": "level volumes of %.0f MiB each: L2-resident; HBM roofline shown for orientation only" % (n_r / 8 / 2**20)},
+        "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3), "clocks": clk,
+        "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
+                "h2d_bytes_per_step": int(hard_h.numel()), "d2h_bytes_per_step": int(16 * 4096 + 32)},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": "reach_level (one level: six maneuver sweeps, copies, transpositions)", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                     "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": lv_ms / max(lv_n, 1), "launches_timed": int(lv_n)},
+        "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
+    }
     p.close()
     replicas.shutdown()
     print(json.dumps(out), flush=True)

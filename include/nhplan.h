@@ -171,6 +171,30 @@ int nhp_run_nturn(nhp_planner *p, int i, int j, int theta, int n_cycles);
  * maneuver with NHP_FLAG_FORWARD_ONLY. */
 int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cycles);
 
+/* Reachability ("bit-vector") planner of appendix C: cost = number of maneuvers, one BIT per pose.
+ * Level volume m holds the poses reachable from the start with <= m maneuvers (bit = 1; layout as C); level m + 1 =
+ * level m OR the sweeps of all maneuvers over level m (l.871, Insert 2 l.873-878); the n_levels + 1 volumes are
+ * kept for back-tracking (l.897).  Uses the collision volume of the last nhp_render_obstacles and none of the costs
+ * (soft volume, ct, dir_mult); NHP_FLAG_FORWARD_ONLY is honoured.  n_levels <= 0 selects 8; at most 254.
+ * The level volumes and three working volumes ((n_levels + 4) N_R / 8 bytes) are allocated by the library at the
+ * first call and reused.  Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_CUDA; a blocked start is reported by
+ * nhp_reach_extract_path. */
+int nhp_reach_run(nhp_planner *p, int i, int j, int theta, int n_levels);
+
+/* Borrowed DEVICE pointer to the level volumes of the last nhp_reach_run: level m starts at word m * N_R / 32. */
+int nhp_reach_levels(nhp_planner *p, const uint32_t **dev_ptr_out, int *n_levels);
+
+/* K[Theta][j][i] (uint8, DEVICE buffer of N_R bytes owned by the caller) = fewest maneuvers that reach the pose = the
+ * first level whose bit is set; 255 = not reached within the levels of the last nhp_reach_run (or blocked). */
+int nhp_reach_count_volume(nhp_planner *p, uint8_t *K_dev);
+
+/* Back-tracking over the level volumes: from the goal at its level k, the maneuvers in cycle order; each walks back
+ * along its curve until a blocked vertex and offers the first vertex reachable with <= k - 1 maneuvers; the first
+ * maneuver with an offer wins (DESIGN R27).  Records as nhp_extract_path; *n_maneuvers = level of the goal.
+ * Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_START_BLOCKED, NHP_E_GOAL_UNREACHED, NHP_E_BUFFER, NHP_E_CUDA. */
+int nhp_reach_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *out_host, int cap, int *count,
+                           int *n_maneuvers);
+
 /* Continue sweeping the existing value volume for n_cycles more cycles. */
 int nhp_run_more(nhp_planner *p, int n_cycles);
 
@@ -229,8 +253,9 @@ long long nhp_launch_count(const nhp_planner *p);
  *   slot 6      collision rendering (a1), slot 7 soft rendering (a2), slot 8 volume init / export (a6),
  *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing,
  *   slot 11     turn-pair launches (RB+RF or LB+next LF in one kernel: two maneuvers per launch)
- *   slot 12     distance transform + soft-image synthesis (nhp_render_obstacles_dt) */
-#define NHP_KERNEL_SLOTS 13
+ *   slot 12     distance transform + soft-image synthesis (nhp_render_obstacles_dt)
+ *   slot 13     one level of the reachability planner (all its launches: copy, six sweeps, transpositions) */
+#define NHP_KERNEL_SLOTS 14
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
 

@@ -17,12 +17,12 @@ ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_
 
 EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_last_error",
            "nhp_render_vehicle_footprint", "nhp_set_box", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
-           "nhp_run_nturn", "nhp_run_nturn_from", "nhp_run_more",
+           "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
-KERNEL_SLOTS = 13
+KERNEL_SLOTS = 14
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
-                     "backtrack", "raster_pack", "turn_pair", "distance_transform")
+                     "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level")
 
 
 class Weights(C.Structure):
@@ -75,6 +75,10 @@ def load_library():
         L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
         L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
         L.nhp_run_nturn_from.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.nhp_reach_run.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
+        L.nhp_reach_levels.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.POINTER(C.c_int)]
+        L.nhp_reach_count_volume.argtypes = [C.c_void_p, C.c_void_p]
+        L.nhp_reach_extract_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Waypoint), C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.nhp_run_more.argtypes = [C.c_void_p, C.c_int]
         L.nhp_cost_volume.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
         L.nhp_extract_path.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.POINTER(Waypoint), C.c_int,
@@ -209,6 +213,23 @@ class Planner:
         """run_nturn with maneuver m0 (0..5 in cycle order, -1 = none) in progress at the start."""
         self._check(self._L.nhp_run_nturn_from(self._h, int(start[0]), int(start[1]), int(start[2]), int(m0), int(n_cycles)),
                     "run_nturn_from")
+
+    def reach_run(self, start, n_levels=8):
+        """Reachability (bit-vector) planner of appendix C: level volumes 0 .. n_levels from `start`."""
+        self._check(self._L.nhp_reach_run(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_levels)), "reach_run")
+
+    def reach_count_numpy(self):
+        """K[theta, j, i] = fewest maneuvers that reach the pose (255 = not within the levels of the last reach_run)."""
+        K = self.torch.empty(self.shape, dtype=self.torch.uint8, device=self.device)
+        self._check(self._L.nhp_reach_count_volume(self._h, K.data_ptr()), "reach_count_volume")
+        return K.cpu().numpy()
+
+    def reach_extract_path(self, goal, cap=4096):
+        buf = (Waypoint * cap)()
+        cnt, nm = C.c_int(0), C.c_int(0)
+        self._check(self._L.nhp_reach_extract_path(self._h, int(goal[0]), int(goal[1]), int(goal[2]), buf, cap,
+                                                   C.byref(cnt), C.byref(nm)), "reach_extract_path")
+        return [(w.i, w.j, w.theta, w.m) for w in buf[:cnt.value]], nm.value
 
     def run_more(self, n_cycles):
         self._check(self._L.nhp_run_more(self._h, int(n_cycles)), "run_more")

@@ -181,6 +181,7 @@ int nhp_planner_destroy(nhp_planner *p)
     cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
     cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
     cudaFree(p->d_status); cudaFree(p->d_plan); cudaFree(p->d_dtg); cudaFree(p->d_goals);
+    cudaFree(p->r_levels); cudaFree(p->r_Lt); cudaFree(p->r_Ct); cudaFree(p->r_Gt);
     if (p->h_status) cudaFreeHost(p->h_status);
     if (p->h_plan) cudaFreeHost(p->h_plan);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
@@ -291,6 +292,64 @@ int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cy
     p->launches += launch_cycles(p, n_cycles);
     CU(cudaGetLastError());
     p->have_run = true;
+    return NHP_OK;
+}
+
+int nhp_reach_run(nhp_planner *p, int i, int j, int theta, int n_levels)
+{
+    if (!p) return NHP_E_ARG;
+    if (!p->have_render) return fail(p, NHP_E_STATE, "reach_run before render_obstacles");
+    if (!in_grid(p, i, j, theta)) return fail(p, NHP_E_ARG, "start pose outside the grid");
+    if (n_levels <= 0) n_levels = 8;
+    if (n_levels > 254) return fail(p, NHP_E_ARG, "more than 254 levels");
+    int k = 0;
+    const int rc = launch_reach_run(p, i, j, theta, n_levels, &k);
+    if (rc != NHP_OK) return fail(p, rc, "allocating the level volumes failed");
+    p->launches += k;
+    p->r_start[0] = i; p->r_start[1] = j; p->r_start[2] = theta;
+    CU(cudaGetLastError());
+    return NHP_OK;
+}
+
+int nhp_reach_levels(nhp_planner *p, const uint32_t **dev_ptr_out, int *n_levels)
+{
+    if (!p || !dev_ptr_out || !n_levels) return fail(p, NHP_E_ARG, "NULL argument");
+    if (p->r_n_levels < 0) return fail(p, NHP_E_STATE, "reach_levels before reach_run");
+    *dev_ptr_out = p->r_levels;
+    *n_levels = p->r_n_levels;
+    return NHP_OK;
+}
+
+int nhp_reach_count_volume(nhp_planner *p, uint8_t *K_dev)
+{
+    if (!p || !K_dev) return fail(p, NHP_E_ARG, "NULL argument");
+    if (p->r_n_levels < 0) return fail(p, NHP_E_STATE, "reach_count_volume before reach_run");
+    if ((uintptr_t)K_dev & 15) return fail(p, NHP_E_BUFFER, "K buffer must be 16-byte aligned");
+    p->launches += launch_reach_count(p, K_dev);
+    CU(cudaGetLastError());
+    return NHP_OK;
+}
+
+int nhp_reach_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *out_host, int cap, int *count, int *n_maneuvers)
+{
+    if (!p || !out_host || !count || !n_maneuvers || cap < 1) return fail(p, NHP_E_ARG, "bad reach_extract_path argument");
+    if (p->r_n_levels < 0) return fail(p, NHP_E_STATE, "reach_extract_path before reach_run");
+    if (!in_grid(p, gi, gj, gtheta)) return fail(p, NHP_E_ARG, "goal pose outside the grid");
+    *count = 0; *n_maneuvers = -1;
+    p->launches += launch_reach_backtrack(p, gi, gj, gtheta);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    const int rc = p->h_status[1];
+    if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
+    if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "goal not reached within the levels of the last reach_run");
+    if (rc != NHP_OK) return fail(p, rc, "plan longer than the internal buffer");
+    const int n = p->h_status[2];
+    if (n > cap) return fail(p, NHP_E_BUFFER, "plan longer than the caller's buffer");
+    std::memcpy(out_host, p->h_plan, sizeof(nhp_waypoint) * n);
+    *count = n;
+    *n_maneuvers = p->h_status[3];
     return NHP_OK;
 }
 

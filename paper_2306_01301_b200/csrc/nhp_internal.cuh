@@ -108,6 +108,10 @@ struct nhp_planner {
     uint8_t *d_Mk = nullptr;       // [levels][n][n]    soft image; level k = max over 2^k columns (soft only)
     bool have_render = false, have_run = false, canonical = false;
     int start[3] = {0, 0, 0};
+    // reachability (bit-vector) planner, reach.cu: level volumes and the transposed working volumes (allocated at the first
+    // nhp_reach_run), number of levels of the last run, its start
+    uint32_t *r_levels = nullptr, *r_Lt = nullptr, *r_Ct = nullptr, *r_Gt = nullptr;
+    int r_cap_levels = 0, r_n_levels = -1, r_start[3] = {0, 0, 0};
     int start_m0 = -1;             // maneuver in progress at the start (nhp_run_nturn_from), -1 = none
     // plan extraction
     int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search: i, j, theta, goal
@@ -161,6 +165,9 @@ int launch_cycles(nhp_planner *p, int n_cycles);
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);     // gi < 0: the goal comes from launch_goal_search
 int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w);
 int launch_seed_in_progress(nhp_planner *p, int m0);
+int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *launches);   // reach.cu
+int launch_reach_backtrack(nhp_planner *p, int gi, int gj, int gt);
+int launch_reach_count(nhp_planner *p, uint8_t *K_dev);
 int launch_straight_tile(nhp_planner *p, int m);      // straight.cu; 0 = not applicable
 int launch_soft_layouts(nhp_planner *p);
 int launch_soft_from_hard(nhp_planner *p, float k, float *dist_dev, int32_t *d2_dev);   // distance.cu: d_hard -> d_soft              // softlayout.cu: S -> S_left, S_right, S_line

@@ -142,6 +142,60 @@ def test_distance_transform_and_soft_image_on_the_device(mods):
     p.close()
 
 
+def test_reachability_planner_of_appendix_c(mods):
+    """Bit-vector planner: fewest-maneuver counts from the level volumes and the plans extracted over
+    them against the oracle, bit for bit, incl. forward-only, N_theta != N and config 2."""
+    oracle, nhp = mods
+    rng = np.random.default_rng(13)
+    cases = [(scenes.random_scene(5, 5, 4, 61, n_rects=5), 12), (scenes.random_scene(6, 5, 5, 62, vehicle=(6, 3), n_rects=12), 6),
+             (scenes.random_scene(5, 7, 4, 63), 5), (scenes.random_scene(6, 6, 8, 64, flags=1), 7), (scenes.random_scene(7, 6, 9, 65, n_rects=30), 4),
+             (scenes.get_config(2), 6)]
+    for sc, n_levels in cases:
+        o, fp = oracle_for(oracle, sc)
+        Cv, _ = o.render(fp, sc.hard, None, method="runs")
+        K = o.reach_run(Cv, sc.start, n_levels)
+        p = nhp.Planner.from_scene(sc) if sc.soft is None else nhp.Planner(sc.log2_n, sc.log2_nt, sc.R, sc.ct, flags=sc.flags & 1)
+        if sc.soft is not None:
+            p.render_vehicle_footprint(sc.mask, sc.ou, sc.ov)
+        p.render_obstacles(sc.hard)
+        p.reach_run(sc.start, n_levels)
+        got = p.reach_count_numpy()
+        assert (got == K).all(), (sc.name, int((got != K).sum()))
+        tj, jj, ij = np.nonzero(K != 255)
+        for k in rng.integers(len(tj), size=30):
+            goal = (int(ij[k]), int(jj[k]), int(tj[k]))
+            assert p.reach_extract_path(goal) == o.reach_backtrack(K, Cv, sc.start, goal), (sc.name, goal)
+        tj, jj, ij = np.nonzero((K == 255) & (Cv == 0))
+        if len(tj):
+            with pytest.raises(nhp.NhpError) as e:
+                p.reach_extract_path((int(ij[0]), int(jj[0]), int(tj[0])))
+            assert e.value.code == -5
+        # a second, shorter run reuses the buffers
+        p.reach_run(sc.start, 2)
+        assert (p.reach_count_numpy() == o.reach_run(Cv, sc.start, 2)).all()
+        p.close()
+
+
+@pytest.mark.slow
+def test_reachability_planner_config3_maze_512(mods):
+    """Full size, the launch configuration `bench.py --reach` times: 20 levels at 512^3."""
+    oracle, nhp = mods
+    sc = scenes.get_config(3)
+    o, fp = oracle_for(oracle, sc)
+    Cv, _ = o.render(fp, sc.hard, None, method="runs")
+    K = o.reach_run(Cv, sc.start, sc.n_cycles)
+    p = nhp.Planner.from_scene(sc)
+    p.render_obstacles(sc.hard)
+    p.reach_run(sc.start, sc.n_cycles)
+    got = p.reach_count_numpy()
+    assert (got == K).all(), int((got != K).sum())
+    far = np.argwhere(K == K[K != 255].max())
+    for t, j, i in far[:: max(1, len(far) // 8)][:8]:
+        goal = (int(i), int(j), int(t))
+        assert p.reach_extract_path(goal) == o.reach_backtrack(K, Cv, sc.start, goal), goal
+    p.close()
+
+
 def test_bounding_box_vehicle_of_appendix_g(mods):
     """nhp_set_box(f, r, s) == the rectangle u in [-r, f), v in [-s, s): collision volume against the
     oracle's brute-force rendering of that rectangle as a mask."""
