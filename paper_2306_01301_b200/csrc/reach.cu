@@ -39,36 +39,38 @@ __device__ __forceinline__ uint32_t ring_carry(const uint2 *sGP, int stride, int
     return c;
 }
 
-// Turn maneuver: CTA = one row of curves y' x all words of x' x S sections of 32 planes.  blockDim = (nw, S).
+// Turn maneuver: CTA = one row of curves y' x all words of x' x S sections of planes.  blockDim = (nw, S).
 template <bool UP>
 __global__ void reach_turn_kernel(uint32_t *__restrict__ Lout, const uint32_t *__restrict__ Lin, const uint32_t *__restrict__ C,
                                   const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
 {
-    extern __shared__ uint2 sGP[];                            // [S][nw] (G, P)
+    extern __shared__ uint2 sGP[];                            // [S][nw] (G, P), then [nt] (first word of the plane's row, bit shift)
     const int n = 1 << log2_n, mx = n - 1, nw = n >> 5, mw = nw - 1, mt = nt - 1, quarter = nt >> 2;
     const int xw = threadIdx.x, sec = threadIdx.y, S = blockDim.y, yp = blockIdx.x;
+    uint2 *sRow = sGP + S * nw;
+    for (int t = sec * nw + xw; t < nt; t += S * nw) {
+        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
+        sRow[t] = make_uint2((uint32_t)((t * n + ((yp + bb) & mx)) * nw), (uint32_t)(ba & mx));
+    }
+    __syncthreads();
     const int t0 = sec * (nt / S), t1 = t0 + nt / S;
     uint32_t v = 0, p = ~0u;
     for (int s = t0; s < t1; s++) {
-        const int t = UP ? s : t0 + t1 - 1 - s;
-        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
-        const size_t row = ((size_t)t * n + ((yp + bb) & mx)) * nw;
-        const int x = (32 * xw + ba) & mx;
-        const uint32_t c = win32(C + row, x, mw);
-        v = (v | win32(Lin + row, x, mw)) & ~c;
+        const uint2 rw = sRow[UP ? s : t0 + t1 - 1 - s];
+        const int x = (32 * xw + (int)rw.y) & mx;
+        const uint32_t c = win32(C + rw.x, x, mw);
+        v = (v | win32(Lin + rw.x, x, mw)) & ~c;
         p &= ~c;
     }
     sGP[sec * nw + xw] = make_uint2(v, p);
     __syncthreads();
     v = ring_carry<UP>(sGP + xw, nw, sec, S);
     for (int s = t0; s < t1; s++) {
-        const int t = UP ? s : t0 + t1 - 1 - s;
-        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];
-        const size_t row = ((size_t)t * n + ((yp + bb) & mx)) * nw;
-        const int x = (32 * xw + ba) & mx;
-        const uint32_t c = win32(C + row, x, mw), r = win32(Lin + row, x, mw);
+        const uint2 rw = sRow[UP ? s : t0 + t1 - 1 - s];
+        const int x = (32 * xw + (int)rw.y) & mx;
+        const uint32_t c = win32(C + rw.x, x, mw), r = win32(Lin + rw.x, x, mw);
         v = (v | r) & ~c;
-        if (v & ~r) or32(Lout + row, x, mw, v & ~r);
+        if (v & ~r) or32(Lout + rw.x, x, mw, v & ~r);
     }
 }
 
@@ -107,7 +109,8 @@ __global__ void reach_rows_kernel(uint32_t *__restrict__ Lout, const uint32_t *_
     }
 }
 
-// 32 x 32 bit-block transpose of the listed slices: dst (row = i, bit = j) from src (row = j, bit = i); ACC: OR into dst
+// 32 x 32 bit-block transpose of the listed slices: dst (row = i, bit = j) from src (row = j, bit = i); ACC: OR into dst.
+// One warp per block, lane = row of the block.
 template <bool ACC>
 __global__ void reach_transpose_kernel(uint32_t *__restrict__ dst, const uint32_t *__restrict__ src, const int16_t *__restrict__ tlist, int log2_n)
 {
@@ -115,11 +118,14 @@ __global__ void reach_transpose_kernel(uint32_t *__restrict__ dst, const uint32_
     const size_t slice = (size_t)tlist[blockIdx.z] * n * nw;
     const int r0 = (blockIdx.y * blockDim.y + threadIdx.y) << 5, wc = blockIdx.x;
     const uint32_t word = src[slice + (size_t)(r0 + lane) * nw + wc];
-    uint32_t mine = 0;
+    // five butterfly stages (swap the off-diagonal j x j blocks of every 2j x 2j block between lanes l and l ^ j)
+    uint32_t mine = word, msk = 0x0000ffffu;
 #pragma unroll
-    for (int k = 0; k < 32; k++) {
-        const uint32_t b = __ballot_sync(0xffffffffu, (word >> k) & 1u);
-        if (lane == k) mine = b;
+    for (int j = 16; j > 0; j >>= 1) {
+        const uint32_t other = __shfl_xor_sync(0xffffffffu, mine, j);
+        if (lane & j) mine ^= ((other >> j) ^ mine) & msk;
+        else mine ^= ((((mine >> j) ^ other) & msk) << j);
+        msk ^= msk << (j >> 1);
     }
     uint32_t *d = dst + slice + (size_t)(32 * wc + lane) * nw + (r0 >> 5);
     if (ACC) { if (mine) *d |= mine; } else *d = mine;
@@ -282,7 +288,7 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
     while (S > 1 && (nw * S > 1024 || nt % S || n % S)) S >>= 1;
     const int trows = n / 32 < 8 ? n / 32 : 8;                  // 32 x 32 blocks per CTA of the transposition
     const dim3 blk(nw, S), tgrid(nw, n / 32 / trows, nx > 0 ? nx : 1), tblk(32, trows);
-    const size_t smem = sizeof(uint2) * (size_t)nw * S;
+    const size_t smem = sizeof(uint2) * (size_t)nw * S, tsmem = smem + sizeof(uint2) * (size_t)nt;
     int k = 0;
     reach_init_kernel<<<(unsigned)((W + 255) / 256), 256, 0, p->stream>>>(p->r_levels, p->C, W, ((size_t)st * n + sj) * n + si, p->d_status);
     if (nx > 0) reach_transpose_kernel<false><<<tgrid, tblk, 0, p->stream>>>(p->r_Ct, p->C, p->d_tlist, p->log2_n);
@@ -293,12 +299,12 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
         uint32_t *Lout = p->r_levels + (size_t)(m + 1) * W;
         cudaMemcpyAsync(Lout, Lin, sizeof(uint32_t) * W, cudaMemcpyDeviceToDevice, p->stream);
         // turn maneuvers, eq (18): LEFT (beta0, beta3), RIGHT (beta2, beta1); LF, RB travel Theta+, LB, RF Theta- (eqs (25)-(28))
-        reach_turn_kernel<true><<<n, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);            // LF
-        reach_turn_kernel<false><<<n, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);           // RF
+        reach_turn_kernel<true><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);            // LF
+        reach_turn_kernel<false><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);           // RF
         k += 3;
         if (!fwd_only) {
-            reach_turn_kernel<false><<<n, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);       // LB
-            reach_turn_kernel<true><<<n, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);        // RB
+            reach_turn_kernel<false><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);       // LB
+            reach_turn_kernel<true><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);        // RB
             k += 2;
         }
         if (ny > 0) {
