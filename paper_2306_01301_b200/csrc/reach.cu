@@ -39,73 +39,113 @@ __device__ __forceinline__ uint32_t ring_carry(const uint2 *sGP, int stride, int
     return c;
 }
 
-// Turn maneuver: CTA = one row of curves y' x all words of x' x S sections of planes.  blockDim = (nw, S).
-template <bool UP>
-__global__ void reach_turn_kernel(uint32_t *__restrict__ Lout, const uint32_t *__restrict__ Lin, const uint32_t *__restrict__ C,
-                                  const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
+// Both maneuvers of one turn family (LF + LB, or RB + RF: the same curves, opposite directions) from ONE pass over the
+// planes: the PL planes of a section are looked up once, (r, c) = (level bits, collision bits) stay in registers, and
+// both directions are summarised and applied from there.  do_up / do_dn select the maneuvers (forward-only vehicles).
+template <int PL>
+__global__ void __launch_bounds__(512, 2) reach_turn2_kernel(uint32_t *__restrict__ Lout, const uint32_t *__restrict__ Lin, const uint32_t *__restrict__ C,
+                                   const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb, int do_up, int do_dn)
 {
-    extern __shared__ uint2 sGP[];                            // [S][nw] (G, P), then [nt] (first word of the plane's row, bit shift)
+    extern __shared__ uint2 sGP[];                            // [S][nw] (G_up, P), [S][nw] (G_dn, P), [nt] plane table
     const int n = 1 << log2_n, mx = n - 1, nw = n >> 5, mw = nw - 1, mt = nt - 1, quarter = nt >> 2;
-    const int xw = threadIdx.x, sec = threadIdx.y, S = blockDim.y, yp = blockIdx.x;
-    uint2 *sRow = sGP + S * nw;
-    for (int t = sec * nw + xw; t < nt; t += S * nw) {
+    const int xl = threadIdx.x, wx = blockDim.x, xw = blockIdx.y * wx + xl, sec = threadIdx.y, S = blockDim.y, yp = blockIdx.x;
+    uint2 *sDn = sGP + S * wx, *sRow = sDn + S * wx;
+    for (int t = sec * wx + xl; t < nt; t += S * wx) {
         const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
         sRow[t] = make_uint2((uint32_t)((t * n + ((yp + bb) & mx)) * nw), (uint32_t)(ba & mx));
     }
     __syncthreads();
-    const int t0 = sec * (nt / S), t1 = t0 + nt / S;
-    uint32_t v = 0, p = ~0u;
-    for (int s = t0; s < t1; s++) {
-        const uint2 rw = sRow[UP ? s : t0 + t1 - 1 - s];
+    uint32_t r[PL], c[PL];
+    uint32_t p = ~0u;
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        const uint2 rw = sRow[sec * PL + k];
         const int x = (32 * xw + (int)rw.y) & mx;
-        const uint32_t c = win32(C + rw.x, x, mw);
-        v = (v | win32(Lin + rw.x, x, mw)) & ~c;
-        p &= ~c;
+        c[k] = win32(C + rw.x, x, mw);
+        r[k] = win32(Lin + rw.x, x, mw);
+        p &= ~c[k];
     }
-    sGP[sec * nw + xw] = make_uint2(v, p);
+    uint32_t vu = 0, vd = 0;
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        vu = (vu | r[k]) & ~c[k];
+        vd = (vd | r[PL - 1 - k]) & ~c[PL - 1 - k];
+    }
+    sGP[sec * wx + xl] = make_uint2(vu, p);
+    sDn[sec * wx + xl] = make_uint2(vd, p);
     __syncthreads();
-    v = ring_carry<UP>(sGP + xw, nw, sec, S);
-    for (int s = t0; s < t1; s++) {
-        const uint2 rw = sRow[UP ? s : t0 + t1 - 1 - s];
-        const int x = (32 * xw + (int)rw.y) & mx;
-        const uint32_t c = win32(C + rw.x, x, mw), r = win32(Lin + rw.x, x, mw);
-        v = (v | r) & ~c;
-        if (v & ~r) or32(Lout + rw.x, x, mw, v & ~r);
+    vu = do_up ? ring_carry<true>(sGP + xl, wx, sec, S) : 0u;
+    vd = do_dn ? ring_carry<false>(sDn + xl, wx, sec, S) : 0u;
+    uint32_t fresh[PL];
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        vu = (vu | r[k]) & ~c[k];
+        fresh[k] = do_up ? vu & ~r[k] : 0u;
+    }
+#pragma unroll
+    for (int k = PL - 1; k >= 0; k--) {
+        vd = (vd | r[k]) & ~c[k];
+        if (do_dn) fresh[k] |= vd & ~r[k];
+        if (fresh[k]) {
+            const uint2 rw = sRow[sec * PL + k];
+            or32(Lout + rw.x, (32 * xw + (int)rw.y) & mx, mw, fresh[k]);
+        }
     }
 }
 
-// Straight maneuver in "rows" form: step = row y of the slice, line x' sits at column (x' + B(y)) & mask, eq (23) with
-// I = 1.  Slices with I = 0 are handled in their transposed copies, where they have exactly this form.
-// CTA = one slice x all words of x' x S sections of rows.  up: travel towards larger y.
-__global__ void reach_rows_kernel(uint32_t *__restrict__ Lout, const uint32_t *__restrict__ Lin, const uint32_t *__restrict__ C,
-                                  const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ, const int16_t *__restrict__ tlist,
-                                  int log2_n, int is_forward)
+// Straight maneuvers SF + SB in "rows" form: step = row y of the slice, line x' sits at column (x' + B(y)) & mask, eq (23)
+// with I = 1.  Slices with I = 0 are handled in their transposed copies, where they have exactly this form.
+// CTA = one slice x all words of x' x S sections of PL rows; both directions from one pass over the rows (as above).
+// The direction of SF is that of growing y iff J(Theta) > 0 (eq (24)); do_rev = 0 drops SB.
+template <int PL>
+__global__ void __launch_bounds__(512, 2) reach_rows2_kernel(uint32_t *__restrict__ Lout, const uint32_t *__restrict__ Lin, const uint32_t *__restrict__ C,
+                                   const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ, const int16_t *__restrict__ tlist,
+                                   int log2_n, int do_rev)
 {
-    extern __shared__ uint2 sGP[];
+    extern __shared__ uint2 sGP[];                            // [S][nw] (G_up, P), [S][nw] (G_dn, P)
     const int n = 1 << log2_n, mx = n - 1, nw = n >> 5, mw = nw - 1;
-    const int xw = threadIdx.x, sec = threadIdx.y, S = blockDim.y, t = tlist[blockIdx.x];
-    const bool up = (is_forward == ((IJ[t] >> 1) & 1));                                     // eq (24)
+    const int xl = threadIdx.x, wx = blockDim.x, xw = blockIdx.y * wx + xl, sec = threadIdx.y, S = blockDim.y, t = tlist[blockIdx.x];
+    const bool fwd_up = ((IJ[t] >> 1) & 1) != 0;
+    const bool do_up = fwd_up || do_rev, do_dn = !fwd_up || do_rev;
     const int16_t *Bt = B + (size_t)t * n;
     const size_t slice = (size_t)t * n * nw;
-    const int y0 = sec * (n / S), y1 = y0 + n / S;
-    uint32_t v = 0, p = ~0u;
-    for (int s = y0; s < y1; s++) {
-        const int y = up ? s : y0 + y1 - 1 - s;
+    uint2 *sDn = sGP + S * wx;
+    uint32_t r[PL], c[PL];
+    uint32_t p = ~0u;
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        const int y = sec * PL + k;
         const int x = (32 * xw + Bt[y]) & mx;
-        const uint32_t c = win32(C + slice + (size_t)y * nw, x, mw);
-        v = (v | win32(Lin + slice + (size_t)y * nw, x, mw)) & ~c;
-        p &= ~c;
+        c[k] = win32(C + slice + (size_t)y * nw, x, mw);
+        r[k] = win32(Lin + slice + (size_t)y * nw, x, mw);
+        p &= ~c[k];
     }
-    sGP[sec * nw + xw] = make_uint2(v, p);
+    uint32_t vu = 0, vd = 0;
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        vu = (vu | r[k]) & ~c[k];
+        vd = (vd | r[PL - 1 - k]) & ~c[PL - 1 - k];
+    }
+    sGP[sec * wx + xl] = make_uint2(vu, p);
+    sDn[sec * wx + xl] = make_uint2(vd, p);
     __syncthreads();
     // (a line is not a ring, but its first cell y' = 0 is wall in both octant classes, so nothing wraps around)
-    v = up ? ring_carry<true>(sGP + xw, nw, sec, S) : ring_carry<false>(sGP + xw, nw, sec, S);
-    for (int s = y0; s < y1; s++) {
-        const int y = up ? s : y0 + y1 - 1 - s;
-        const int x = (32 * xw + Bt[y]) & mx;
-        const uint32_t c = win32(C + slice + (size_t)y * nw, x, mw), r = win32(Lin + slice + (size_t)y * nw, x, mw);
-        v = (v | r) & ~c;
-        if (v & ~r) or32(Lout + slice + (size_t)y * nw, x, mw, v & ~r);
+    vu = do_up ? ring_carry<true>(sGP + xl, wx, sec, S) : 0u;
+    vd = do_dn ? ring_carry<false>(sDn + xl, wx, sec, S) : 0u;
+    uint32_t fresh[PL];
+#pragma unroll
+    for (int k = 0; k < PL; k++) {
+        vu = (vu | r[k]) & ~c[k];
+        fresh[k] = do_up ? vu & ~r[k] : 0u;
+    }
+#pragma unroll
+    for (int k = PL - 1; k >= 0; k--) {
+        vd = (vd | r[k]) & ~c[k];
+        if (do_dn) fresh[k] |= vd & ~r[k];
+        if (fresh[k]) {
+            const int y = sec * PL + k;
+            or32(Lout + slice + (size_t)y * nw, (32 * xw + Bt[y]) & mx, mw, fresh[k]);
+        }
     }
 }
 
@@ -284,11 +324,20 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
     }
     const bool fwd_only = p->w.flags & NHP_FLAG_FORWARD_ONLY;
     const int nx = p->n_xslices, ny = nt - nx;
-    int S = 32;                                                 // sections per curve: whole planes / rows per section, <= 1024 threads per CTA
-    while (S > 1 && (nw * S > 1024 || nt % S || n % S)) S >>= 1;
     const int trows = n / 32 < 8 ? n / 32 : 8;                  // 32 x 32 blocks per CTA of the transposition
-    const dim3 blk(nw, S), tgrid(nw, n / 32 / trows, nx > 0 ? nx : 1), tblk(32, trows);
-    const size_t smem = sizeof(uint2) * (size_t)nw * S, tsmem = smem + sizeof(uint2) * (size_t)nt;
+    const dim3 tgrid(nw, n / 32 / trows, nx > 0 ? nx : 1), tblk(32, trows);
+    // sweeps: 16 planes (rows) per thread, as many words of curves per CTA as fit 512 threads (sections of different words
+    // do not talk to each other); 32 planes per thread only when a curve has more than 512 x 16 of them
+    auto geom = [&](int len, int &PL, dim3 &blk, int &wgrid, size_t &smem, int table) {
+        PL = (len / 16 <= 512) ? 16 : 32;
+        const int S = len / PL;
+        int wx = 512 / S; if (wx > nw) wx = nw; if (wx < 1) wx = 1;
+        blk = dim3(wx, S); wgrid = nw / wx;
+        smem = sizeof(uint2) * ((size_t)2 * wx * S + table);
+    };
+    int PLn, PLr, tw, rw; dim3 tblk2, rblk2; size_t t2smem, r2smem;
+    geom(nt, PLn, tblk2, tw, t2smem, nt);
+    geom(n, PLr, rblk2, rw, r2smem, 0);
     int k = 0;
     reach_init_kernel<<<(unsigned)((W + 255) / 256), 256, 0, p->stream>>>(p->r_levels, p->C, W, ((size_t)st * n + sj) * n + si, p->d_status);
     if (nx > 0) reach_transpose_kernel<false><<<tgrid, tblk, 0, p->stream>>>(p->r_Ct, p->C, p->d_tlist, p->log2_n);
@@ -299,26 +348,26 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
         uint32_t *Lout = p->r_levels + (size_t)(m + 1) * W;
         cudaMemcpyAsync(Lout, Lin, sizeof(uint32_t) * W, cudaMemcpyDeviceToDevice, p->stream);
         // turn maneuvers, eq (18): LEFT (beta0, beta3), RIGHT (beta2, beta1); LF, RB travel Theta+, LB, RF Theta- (eqs (25)-(28))
-        reach_turn_kernel<true><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);            // LF
-        reach_turn_kernel<false><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);           // RF
-        k += 3;
-        if (!fwd_only) {
-            reach_turn_kernel<false><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3);       // LB
-            reach_turn_kernel<true><<<n, blk, tsmem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1);        // RB
-            k += 2;
+        if (PLn == 16) {
+            reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3, 1, !fwd_only);   // LF (+ LB)
+            reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1, !fwd_only, 1);   // RF (+ RB)
+        } else {
+            reach_turn2_kernel<32><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3, 1, !fwd_only);
+            reach_turn2_kernel<32><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1, !fwd_only, 1);
         }
+        k += 3;
         if (ny > 0) {
-            reach_rows_kernel<<<ny, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, 1);
-            if (!fwd_only) reach_rows_kernel<<<ny, blk, smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, 0);
-            k += fwd_only ? 1 : 2;
+            if (PLr == 16) reach_rows2_kernel<16><<<dim3(ny, rw), rblk2, r2smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, !fwd_only);
+            else reach_rows2_kernel<32><<<dim3(ny, rw), rblk2, r2smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, !fwd_only);
+            k += 1;
         }
         if (nx > 0) {
             reach_transpose_kernel<false><<<tgrid, tblk, 0, p->stream>>>(p->r_Lt, Lin, p->d_tlist, p->log2_n);
             cudaMemsetAsync(p->r_Gt, 0, sizeof(uint32_t) * W, p->stream);
-            reach_rows_kernel<<<nx, blk, smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, 1);
-            if (!fwd_only) reach_rows_kernel<<<nx, blk, smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, 0);
+            if (PLr == 16) reach_rows2_kernel<16><<<dim3(nx, rw), rblk2, r2smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, !fwd_only);
+            else reach_rows2_kernel<32><<<dim3(nx, rw), rblk2, r2smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, !fwd_only);
             reach_transpose_kernel<true><<<tgrid, tblk, 0, p->stream>>>(Lout, p->r_Gt, p->d_tlist, p->log2_n);
-            k += fwd_only ? 4 : 5;
+            k += 4;
         }
     }
     p->r_n_levels = n_levels;
