@@ -67,6 +67,17 @@ struct RelaxLoop<UP, SOFT, 32> {
     static __device__ __forceinline__ void run(uint32_t *, uint32_t &, uint32_t &, uint32_t, uint32_t, const uint4 &, const uint4 &, uint32_t &) {}
 };
 
+// Warp-uniform short cut (data-dependent, same result): nothing finite travels into this tile on any of the 32 lines
+// (t >= VI_INF; every such value acts alike) and no vertex of the tile holds a finite value (v - 1 wraps blocked
+// vertices to 2^32 - 1 and is >= 2^30 for unreached ones): the relaxation cannot change anything.
+__device__ __forceinline__ bool tile_is_idle(const uint32_t (&u)[32], uint32_t t)
+{
+    uint32_t lowest = 0xffffffffu;
+#pragma unroll
+    for (int k = 0; k < 32; k++) lowest = __viaddmin_u32(u[k], 0xffffffffu, lowest);
+    return __all_sync(0xffffffffu, t >= VI_INF && lowest >= VI_INF - 1u);
+}
+
 // ---------------------------------------------------------------------------------------------
 // Slices with I = 0 (|tan| <= 1, eq (19)): the sweep step is the COLUMN i and line x' sits at row
 // (x' + B(i)) & mask, eq (23): the lines run along the memory-fast axis, so "thread = line" needs a transposition
@@ -224,7 +235,8 @@ __device__ __forceinline__ void xr_band_sweep(uint32_t *__restrict__ Vslice, con
             s0 = sl[lane]; s1 = sl[32 + lane];
         }
         uint32_t cm = 0;
-        if (up) RelaxLoop<true, SOFT>::run(u, t, wp, w, ct, s0, s1, cm);
+        if (tile_is_idle(u, t)) { }
+        else if (up) RelaxLoop<true, SOFT>::run(u, t, wp, w, ct, s0, s1, cm);
         else RelaxLoop<false, SOFT>::run(u, t, wp, w, ct, s0, s1, cm);
         const uint32_t lines = __ballot_sync(0xffffffffu, cm != 0u);
         if (lines) {
@@ -301,7 +313,8 @@ __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restr
         uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
         if (SOFT) { s0 = ld_nc16(Sl + 32 * T); s1 = ld_nc16(Sl + 32 * T + 16); }
         uint32_t cm = 0;
-        if (up) RelaxLoop<true, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
+        if (tile_is_idle(u, tv)) { }
+        else if (up) RelaxLoop<true, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
         else RelaxLoop<false, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
         if (__any_sync(0xffffffffu, cm != 0u)) {
 #pragma unroll

@@ -301,9 +301,12 @@ struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4
 //                 configuration space, ~20 % of the warps in configs 3 and 4): the section passes nothing on
 //                 (M = infinity, D = D_CAP) and has nothing to update
 //   none_blocked  no vertex is blocked (~16 %): the chains run without the nhp_gate op
+//   no_finite     (hard costs only) no vertex of the warp holds a finite value yet: the section generates nothing
+//                 (M = infinity, D as always), and if no finite value arrives either, the apply pass has nothing to do
+// Returns true iff the apply pass ran (the vertices may have changed).
 template <int L, bool UP, bool SOFT, bool CS_AFTER>
-__device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
-                                              bool all_blocked, bool none_blocked, uint2 *sMD, int sec, int S, int lane,
+__device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
+                                              bool all_blocked, bool none_blocked, bool &no_finite, uint2 *sMD, int sec, int S, int lane,
                                               unsigned long long &after, uint32_t one)
 {
     if (all_blocked) {
@@ -311,7 +314,23 @@ __device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
         sMD[sec * 32 + lane] = md;
         sMD[(sec + S) * 32 + lane] = md;
         __syncthreads();
-        return;
+        return false;
+    }
+    if (!SOFT && no_finite) {
+        const bool ia = UP ? blocked_lo : blocked_hi, ib = UP ? blocked_hi : blocked_lo;
+        const uint32_t dh = (uint32_t)(L / 2) * pass.w;
+        const uint2 md = make_uint2(0x7fffffffu, (ia || ib) ? D_CAP : 2 * dh);
+        sMD[sec * 32 + lane] = md;
+        sMD[(sec + S) * 32 + lane] = md;
+        __syncthreads();
+        uint32_t ta = ripple_carry<UP>(sMD, sec, S, lane);
+        if (__all_sync(0xffffffffu, ta >= VI_INF)) return false;                 // nothing arrives: nothing changes
+        // something arrives: the ordinary apply pass (M of H0 is infinite, so the carry into H1 is ta + D(H0))
+        uint32_t tb = __viaddmin_u32(ta, ia ? D_CAP : dh, 0x7fffffffu), wa = pass.w, wb = pass.w;
+        sw.len = pass.w;
+        SecLoop<L, UP, SOFT, CS_AFTER, true>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
+        no_finite = false;
+        return true;
     }
     const bool ia = UP ? blocked_lo : blocked_hi, ib = UP ? blocked_hi : blocked_lo;     // H0, H1 in travel order
     sw.len = pass.w;
@@ -334,6 +353,7 @@ __device__ __forceinline__ void turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
     wa = wb = SOFT ? 0u : sw.len;
     if (none_blocked) SecLoop<L, UP, SOFT, CS_AFTER, false>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
     else SecLoop<L, UP, SOFT, CS_AFTER, true>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
+    return true;
 }
 
 // Row addressing of a tile: so[t] = element index of the tile's first vertex in plane t (row base + first column).
@@ -416,9 +436,27 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     const bool all_blocked = __all_sync(0xffffffffu, before == 0ull);
     // (soft kernels keep one chain variant: a second copy of their loops costs registers they do not have)
     const bool none_blocked = !SOFT && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
-    turn_maneuver<L, UP0, SOFT, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, sMD, sec, S, lane, after, one);
-    if (NPASS == 2) turn_maneuver<L, !UP0, SOFT, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, sMD + 2 * S * 32, sec, S, lane, after, one);
-    if (all_blocked) after = before;
+    // "no finite value in this warp yet": min over (v - 1) with wrap-around (blocked 0 -> 2^32 - 1, unreached -> 2^30)
+    bool no_finite = false;
+    if (!SOFT) {
+        uint32_t lowest = 0xffffffffu;
+#pragma unroll
+        for (int k = 0; k < L; k++) lowest = __viaddmin_u32(col[k], 0xffffffffu, lowest);
+        no_finite = __all_sync(0xffffffffu, lowest >= VI_INF - 1u);
+    }
+    const bool ran_a = turn_maneuver<L, UP0, SOFT, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
+                                                                lane, after, one);
+    bool ran_last = ran_a;
+    if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, SOFT, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
+                                                                  sMD + 2 * S * 32, sec, S, lane, after, one);
+    if (!ran_last) {                                          // the "after" sum lives in the last apply pass: take it here if that pass did not run
+        after = before;
+        if (NPASS == 2 && ran_a) {
+            after = 0;
+#pragma unroll
+            for (int k = 0; k < L; k++) checksum_add(after, col[k], one);
+        }
+    }
     if (after != before) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills
