@@ -262,6 +262,20 @@ class Oracle:
             raise OracleError(rc, "dijkstra")
         return V
 
+    def graph_size_at(self, Cv, Sv, start, cell, kind="star"):
+        """(vertices settled, edges relaxed) at `cell` = (i, j, theta) by one Dijkstra run: k_V, k_E of Table 1."""
+        L = _load()
+        L.orc_dijkstra_probe.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int]
+        L.orc_dijkstra_probe_result.argtypes = [C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.orc_dijkstra_probe(self._h, cell[0], cell[1], cell[2])
+        try:
+            self.dijkstra(Cv, Sv, start, kind)
+            kv, ke = C.c_int(0), C.c_int(0)
+            L.orc_dijkstra_probe_result(C.byref(kv), C.byref(ke))
+        finally:
+            L.orc_dijkstra_probe(self._h, -1, -1, -1)
+        return kv.value, ke.value
+
     def backtrack(self, V, Cv, Sv, start, goal, cap=4096):
         self._vols(V, Cv, Sv)
         out = (_Waypoint * cap)()

@@ -17,8 +17,10 @@
  *                   (Lemma 4/5 l.779-785), curve maps are bijections (l.224,269,302)
  *   edge maps ..... LB o LF = id etc., edge(p) = curve-map(step+1)             (l.306, l.320)
  *   sweeps ........ closed form on one curve, fix-point == Star Dijkstra == Compact Dijkstra,
- *                   layered brute-force DP on tiny grids, Dubins / Reeds-Shepp closed forms
- *                   within Theorem 1's bounds, 26-neighbour Piano-mover relaxation (l.88)
+ *                   layered brute-force DP on tiny grids, 26-neighbour Piano-mover relaxation (l.88);
+ *                   free-space fix-point against the Dubins / Reeds-Shepp closed forms within the bounds of
+ *                   Theorems 1, 6, 7 (l.104, 809, 815): tests/test_oracle_reeds_shepp.py, tests/closed_forms.py
+ *   graph sizes ... k_V / k_E of Table 1 (l.427) counted on the Dijkstra itself (tests/test_oracle_tables.py)
  *   render ........ brute force vs exact box dilation at axis angles; run renderer vs brute force
  *   back-track .... plan is a valid chain of curve segments whose cost sums to the reported cost
  *   orc_render_*'s footprint rasterisation rule (DESIGN R15) is OUR definition: "parity
@@ -517,6 +519,18 @@ static hitem hpop(heap *h)
     return top;
 }
 
+/* Instrumentation for the structural pin of Table 1 (k_V vertices and k_E edges per X):
+ * while a probe cell is set, the next Dijkstra run counts the vertices of that cell it settles and the edges it relaxes
+ * out of them.  Counting only: the search itself is untouched. */
+static size_t g_probe_X = (size_t)-1;
+static int g_probe_vertices = 0, g_probe_edges = 0;
+void orc_dijkstra_probe(const orc_ctx *c, int i, int j, int t)
+{
+    g_probe_X = (i < 0) ? (size_t)-1 : ((size_t)t * c->n + j) * c->n + i;
+    g_probe_vertices = g_probe_edges = 0;
+}
+void orc_dijkstra_probe_result(int *vertices, int *edges) { *vertices = g_probe_vertices; *edges = g_probe_edges; }
+
 int orc_dijkstra_from(const orc_ctx *c, int kind, const uint8_t *C, const uint8_t *S, int si, int sj, int st, int m0, uint32_t *Vout)
 {
     int n = c->n, nt = c->nt;
@@ -537,11 +551,13 @@ int orc_dijkstra_from(const orc_ctx *c, int kind, const uint8_t *C, const uint8_
         D[sidx * nv + 1 + m0] = 0;
         hpush(&h, 0, (uint64_t)sidx * nv + 1 + m0);
     }
-#define RELAX(vid, nd) do { uint32_t nd_ = (nd); uint64_t v_ = (vid); if (nd_ < D[v_]) { D[v_] = nd_; hpush(&h, nd_, v_); } } while (0)
+#define RELAX(vid, nd) do { uint32_t nd_ = (nd); uint64_t v_ = (vid); g_probe_edges += probing; if (nd_ < D[v_]) { D[v_] = nd_; hpush(&h, nd_, v_); } } while (0)
     while (h.n) {
         hitem it = hpop(&h);
         if (it.d != D[it.v]) continue;
         size_t X = it.v / nv; int k = (int)(it.v % nv);
+        const int probing = (X == g_probe_X);
+        g_probe_vertices += probing;
         int i = (int)(X % n), j = (int)((X / n) % n), t = (int)(X / ((size_t)n * n));
         if (kind == 0) {
             if (k == 0) {                                   /* transition vertex: T -> (X,m), cost ct[m] */

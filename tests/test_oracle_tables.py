@@ -159,3 +159,21 @@ def test_turn_directions_match_the_continuum_model():
             # six steps of length ~2 pi R / N_theta (turn) or 1/max(|cos|,|sin|) (straight) along +-heading
             assert sgn * float(d @ heading) > 1.5
             assert abs(float(d @ np.array([-heading[1], heading[0]]))) < 1.6
+
+
+def test_graph_sizes_of_table_1():
+    """PAPER.md:427 and Table 1 l.436-437: the Star graph has k_V = 7 vertices and k_E = 18 edges per configuration X,
+    the Compact graph 3 and 10 (tests/golden/paper_constants.txt).  Counted on the oracle's own Dijkstra at an interior
+    cell of free space: the vertices of X it settles and the edges it relaxes out of them."""
+    ct = (4096, 0, 5000, 5000, 0, 4096)                          # conforming weights, so that both graphs apply
+    o = oracle.Oracle(5, 5, 4, ct)
+    fp = oracle.Footprint(np.ones((1, 1), np.uint8), 0.0, 0.0)
+    C, _ = o.render(fp, np.zeros((32, 32), np.uint8))
+    for cell in ((16, 16, 3), (9, 20, 30)):
+        assert o.graph_size_at(C, None, (12, 12, 0), cell, "star") == (GOLD["kV_star"], GOLD["kE_star"])
+        assert o.graph_size_at(C, None, (12, 12, 0), cell, "compact") == (GOLD["kV_compact"], GOLD["kE_compact"])
+    # the Piano-mover's graph of the comparison: one vertex, six neighbours (tests/helpers.py uses its 26-neighbour relaxation)
+    assert (GOLD["kV_piano"], GOLD["kE_piano"]) == (1, 6)
+    # forward only: the three reverse maneuver vertices and their edges disappear (Dubins car, PAPER.md:681)
+    of = oracle.Oracle(5, 5, 4, ct, flags=oracle.FLAG_FORWARD_ONLY)
+    assert of.graph_size_at(C, None, (12, 12, 0), (16, 16, 3), "star") == (4, 9)
