@@ -9,9 +9,11 @@
  *   obstacle image -> [nhp_render_obstacles: steps 3-4] -> [nhp_run_nturn: step 5]
  *   -> [nhp_extract_path: steps 6-8] -> plan on the host.
  * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.  The library
- * never allocates after nhp_planner_create ("no memory allocation takes place during processing",
- * PAPER.md:565) and enqueues all work on the caller's stream; only nhp_extract_path, nhp_status and
- * nhp_debug_tables synchronise that stream.
+ * allocates device memory in nhp_planner_create only ("no memory allocation takes place during processing",
+ * PAPER.md:565): the large buffers are the caller's (nhp_buffers, sized by nhp_query_sizes from the grid and the
+ * nhp_limits), the small tables are the library's.  All work is enqueued on the caller's stream; only the
+ * nhp_extract_path family, nhp_render_vehicle_footprint, nhp_status, nhp_kernel_times and the debug accessors
+ * synchronise that stream.  Every entry point makes the handle's device current for the duration of the call.
  *
  * Grid: N x N spatial cells (N = 2^log2_n) and N_theta = 2^log2_ntheta headings,
  * Theta <-> angle 2 pi Theta / N_theta, all indices taken modulo their dimension, one-cell hard wall
@@ -46,6 +48,12 @@ extern "C" {
 #define NHP_FLAG_SOFT 2           /* a soft-cost volume S is rendered and used */
 #define NHP_FLAG_SIMPLE_KERNELS 4 /* thread-per-curve bring-up kernels (the paper's own mapping, l.356);
                                      same results, kept for A/B measurements */
+#define NHP_FLAG_FIXED_WORK 8     /* switch off the data-dependent short cuts of the sweeps (warps whose vertices are all
+                                     blocked / hold no finite value yet skip their chains): every launch then executes
+                                     the same instructions whatever the scene holds ("run time independent of scene",
+                                     PAPER.md:39, l.565).  Same results; for measuring the fixed-work time */
+
+#define NHP_DEFAULT_CYCLES 8      /* PAPER.md:392 "our default is 8 cycles" (n_cycles <= 0 selects it) */
 
 /* error codes (all entry points return 0 on success) */
 #define NHP_OK 0
@@ -78,9 +86,22 @@ typedef struct nhp_sizes {
     size_t V_bytes;          /* value volume, uint32 per vertex            (one volume) */
     size_t C_bytes;          /* collision volume, 1 bit per vertex             */
     size_t S_bytes;          /* soft volume, uint8 per vertex; 0 without NHP_FLAG_SOFT  */
-    size_t workspace_bytes;  /* 3 N_R bytes with NHP_FLAG_SOFT (curve-major copies of S for the left-turn, right-turn
-                                and straight sweeps, written by nhp_render_obstacles), else 0                     */
+    size_t workspace_bytes;  /* everything else that scales with the grid or the limits: the footprint tables (E_Theta
+                                bitmaps, run lists, sparse tables of the image rows), with NHP_FLAG_SOFT the curve-major
+                                copies of S for the left-turn, right-turn and straight sweeps (3 N_R bytes), with
+                                max_reach_levels > 0 the level volumes of the reachability planner
+                                ((max_reach_levels + 4) N_R / 8 bytes)                                            */
 } nhp_sizes;
+
+/* Upper bounds fixed at creation so that nothing is allocated afterwards.  A NULL pointer or a zero field
+ * selects the default. */
+typedef struct nhp_limits {
+    int32_t max_footprint_radius;  /* largest circumscribed radius of a vehicle mask around its origin, cells (+2 for Psi and
+                                      rounding); default min(64, N/2 - 1).  nhp_render_vehicle_footprint / nhp_set_box
+                                      fail with NHP_E_BUFFER beyond it */
+    int32_t max_reach_levels;      /* largest n_levels of nhp_reach_run; default 0 = the reachability planner is not used
+                                      (nhp_reach_run then fails with NHP_E_BUFFER) */
+} nhp_limits;
 
 /* Caller-owned DEVICE buffers (e.g. torch tensors), 256-byte aligned, alive until nhp_planner_destroy. */
 typedef struct nhp_buffers {
@@ -96,17 +117,20 @@ typedef struct nhp_waypoint {
     int32_t i, j, theta, m;
 } nhp_waypoint;
 
-/* Sizes of the caller-owned buffers for a grid.  Pure host arithmetic. */
-int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, nhp_sizes *out);
+/* Sizes of the caller-owned buffers for a grid and its limits (lim may be NULL).  Pure host arithmetic. */
+int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, const nhp_limits *lim, nhp_sizes *out);
 
 /* ini(R, cT, Lx, Lt) of PAPER.md:1169.  Builds the integer tables of section V.C (beta, Psi, B, I, J,
  * edge lengths) on the host in fp64 once and uploads them.
  *   R_cells      minimum turn radius in cells, >= 1; N_theta >= 2 pi R is enforced
+ *   lim          the limits the buffers were sized for (NULL = defaults), see nhp_limits
  *   dev          caller-owned device buffers (see nhp_buffers); S may be NULL without NHP_FLAG_SOFT
- *   cuda_stream  a cudaStream_t (0 = legacy default stream) on the current device
+ *   cuda_stream  a cudaStream_t (0 = legacy default stream) on the device that owns dev->V; that device is made
+ *                current inside every call on the handle
+ * This is the only call that allocates device memory (the small tables, a few hundred KB).
  * Errors: NHP_E_ARG, NHP_E_NOT_POW2, NHP_E_ANGRES, NHP_E_WEIGHTS, NHP_E_BUFFER, NHP_E_CUDA. */
 int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_cells,
-                       const nhp_weights *w, const nhp_buffers *dev, void *cuda_stream);
+                       const nhp_weights *w, const nhp_limits *lim, const nhp_buffers *dev, void *cuda_stream);
 
 int nhp_planner_destroy(nhp_planner *p);
 
@@ -121,7 +145,9 @@ const char *nhp_last_error(const nhp_planner *p);
  * Rasterises, per Theta, the set E_Theta of image-pixel offsets covered by the footprint of a pose
  * (DESIGN R15: a pixel is covered iff its centre, rotated into the vehicle frame with Q14 integer
  * cos/sin, falls in a set mask pixel; the half-cell pose offset Psi of eq (16) is applied, l.259).
- * The footprint's circumscribed radius must be < N/2 - 2.  Errors: NHP_E_ARG, NHP_E_CUDA. */
+ * The footprint's circumscribed radius (+2) must be <= nhp_limits.max_footprint_radius and < N/2, and an arbitrary
+ * mask may break into at most 4 runs per footprint row on average (the run lists live in the caller's workspace).
+ * Synchronises the stream (mask_host may be freed on return).  Errors: NHP_E_ARG, NHP_E_BUFFER, NHP_E_CUDA. */
 int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int mw, int mh,
                                  double origin_u, double origin_v);
 
@@ -176,9 +202,8 @@ int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cy
  * level m OR the sweeps of all maneuvers over level m (l.871, Insert 2 l.873-878); the n_levels + 1 volumes are
  * kept for back-tracking (l.897).  Uses the collision volume of the last nhp_render_obstacles and none of the costs
  * (soft volume, ct, dir_mult); NHP_FLAG_FORWARD_ONLY is honoured.  n_levels <= 0 selects 8; at most 254.
- * The level volumes and three working volumes ((n_levels + 4) N_R / 8 bytes) are allocated by the library at the
- * first call and reused.  Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_CUDA; a blocked start is reported by
- * nhp_reach_extract_path. */
+ * The level volumes and three working volumes live in the caller's workspace: n_levels <= nhp_limits.max_reach_levels.
+ * Errors: NHP_E_ARG, NHP_E_STATE, NHP_E_BUFFER, NHP_E_CUDA; a blocked start is reported by nhp_reach_extract_path. */
 int nhp_reach_run(nhp_planner *p, int i, int j, int theta, int n_levels);
 
 /* Borrowed DEVICE pointer to the level volumes of the last nhp_reach_run: level m starts at word m * N_R / 32. */
@@ -241,12 +266,21 @@ int nhp_pose_to_index(const nhp_planner *p, double x, double y, double theta_rad
 int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t *B, uint8_t *I, int8_t *J,
                      uint32_t *len_q);
 
+/* Debug accessor: the structuring elements E_Theta of the current footprint (DESIGN R15) -> HOST.
+ *   *radius   receives rad; the elements are (2 rad + 1) x (2 rad + 1) offset windows
+ *   covered   HOST uint8 [N_theta][2 rad + 1][2 rad + 1] or NULL (size query): covered[Theta][db + rad][da + rad] = 1 iff
+ *             the footprint of a pose of heading Theta covers the image pixel (i + da, j + db)
+ *   cap       bytes available at `covered`
+ * Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_BUFFER, NHP_E_CUDA. */
+int nhp_debug_footprint(nhp_planner *p, int *radius, uint8_t *covered, size_t cap);
+
 /* Number of kernels launched by this handle since creation (for bench.py's gpu_launches). */
 long long nhp_launch_count(const nhp_planner *p);
 
 /* Per-kernel device timing for bench.py's roofline line.  With profiling enabled every kernel launch of the
- * handle is bracketed by a cudaEvent pair recorded on the handle's stream (up to 1024 launches between two
- * reads; further launches run untimed).  nhp_kernel_times synchronises the stream, adds the elapsed times
+ * handle is bracketed by a cudaEvent pair recorded on the handle's stream (the pool of events grows as needed, up to
+ * 65536 launches between two reads; launches beyond that run untimed and are counted by nhp_prof_dropped).
+ * nhp_kernel_times synchronises the stream, adds the elapsed times
  * of the pairs recorded since the last read to running sums, copies the sums to HOST arrays of
  * NHP_KERNEL_SLOTS entries and, with reset != 0, zeroes them.
  *   slots 0..5  maneuver kernels in cycle order (LF, SF, RB, RF, SB, LB)
@@ -258,6 +292,8 @@ long long nhp_launch_count(const nhp_planner *p);
 #define NHP_KERNEL_SLOTS 14
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
+/* Launches that ran untimed since creation because the event pool was exhausted (0 in any sane use). */
+long long nhp_prof_dropped(const nhp_planner *p);
 
 #ifdef __cplusplus
 }

@@ -10,7 +10,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libnhplan.so")
 
 INF = 0xFFFFFFFF
-FLAG_FORWARD_ONLY, FLAG_SOFT, FLAG_SIMPLE_KERNELS = 1, 2, 4
+FLAG_FORWARD_ONLY, FLAG_SOFT, FLAG_SIMPLE_KERNELS, FLAG_FIXED_WORK = 1, 2, 4, 8
+DEFAULT_CYCLES = 8                                          # NHP_DEFAULT_CYCLES
+PLAN_EAGER = 128                                            # waypoints that come back with the status words (NHP_PLAN_EAGER)
 MANEUVER_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB")
 ERRORS = {-1: "NHP_E_ARG", -2: "NHP_E_NOT_POW2", -3: "NHP_E_ANGRES", -4: "NHP_E_START_BLOCKED",
           -5: "NHP_E_GOAL_UNREACHED", -6: "NHP_E_BUFFER", -7: "NHP_E_CUDA", -8: "NHP_E_STATE", -9: "NHP_E_WEIGHTS"}
@@ -19,7 +21,7 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_render_vehicle_footprint", "nhp_set_box", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
-           "nhp_debug_tables", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times")
+           "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped")
 KERNEL_SLOTS = 14
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
                      "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level")
@@ -31,6 +33,10 @@ class Weights(C.Structure):
 
 class Sizes(C.Structure):
     _fields_ = [("V_bytes", C.c_size_t), ("C_bytes", C.c_size_t), ("S_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
+
+
+class Limits(C.Structure):
+    _fields_ = [("max_footprint_radius", C.c_int32), ("max_reach_levels", C.c_int32)]
 
 
 class Buffers(C.Structure):
@@ -62,9 +68,9 @@ def load_library():
             raise ImportError(f"{_LIB_PATH} is missing: run `python -m paper_2306_01301_b200.build` "
                               "(or __graft_entry__.build()); there is no CPU fallback")
         L = C.CDLL(_LIB_PATH)
-        L.nhp_query_sizes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Sizes)]
+        L.nhp_query_sizes.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(Limits), C.POINTER(Sizes)]
         L.nhp_planner_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_int, C.c_double, C.POINTER(Weights),
-                                         C.POINTER(Buffers), C.c_void_p]
+                                         C.POINTER(Limits), C.POINTER(Buffers), C.c_void_p]
         L.nhp_planner_destroy.argtypes = [C.c_void_p]
         L.nhp_last_error.argtypes = [C.c_void_p]
         L.nhp_last_error.restype = C.c_char_p
@@ -89,6 +95,9 @@ def load_library():
         L.nhp_index_to_pose.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int] + [C.POINTER(C.c_double)] * 3
         L.nhp_pose_to_index.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double] + [C.POINTER(C.c_int)] * 3
         L.nhp_debug_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        L.nhp_debug_footprint.argtypes = [C.c_void_p, C.POINTER(C.c_int), C.c_void_p, C.c_size_t]
+        L.nhp_prof_dropped.argtypes = [C.c_void_p]
+        L.nhp_prof_dropped.restype = C.c_longlong
         L.nhp_launch_count.argtypes = [C.c_void_p]
         L.nhp_launch_count.restype = C.c_longlong
         L.nhp_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -97,9 +106,10 @@ def load_library():
     return _lib
 
 
-def query_sizes(log2_n, log2_ntheta, flags=0):
+def query_sizes(log2_n, log2_ntheta, flags=0, max_footprint_radius=0, max_reach_levels=0):
     s = Sizes()
-    rc = load_library().nhp_query_sizes(log2_n, log2_ntheta, flags, C.byref(s))
+    lim = Limits(max_footprint_radius, max_reach_levels)
+    rc = load_library().nhp_query_sizes(log2_n, log2_ntheta, flags, C.byref(lim), C.byref(s))
     if rc:
         raise NhpError(rc, "query_sizes")
     return s
@@ -109,7 +119,9 @@ class Planner:
     """One planner handle = one grid, one stream.  Method names follow the C ABI without the nhp_ prefix."""
 
     def __init__(self, log2_n, log2_ntheta, R, ct, dir_mult=(256,) * 6, cost_one_log2=10, flags=0, device="cuda:0",
-                 stream=None):
+                 stream=None, max_footprint_radius=0, reach_levels=0):
+        """max_footprint_radius / reach_levels: the nhp_limits the workspace is sized for (0 = the library's defaults:
+        radius min(64, N/2 - 1), no reachability planner)."""
         import torch
         self._L = load_library()
         if not torch.cuda.is_available():
@@ -119,18 +131,18 @@ class Planner:
         self.n, self.nt = 1 << log2_n, 1 << log2_ntheta
         self.shape = (self.nt, self.n, self.n)
         self.flags = flags
-        sz = query_sizes(log2_n, log2_ntheta, flags)
+        sz = query_sizes(log2_n, log2_ntheta, flags, max_footprint_radius, reach_levels)
         with torch.cuda.device(self.device):
             self.V = torch.empty(sz.V_bytes // 4, dtype=torch.int32, device=self.device)
             self.C = torch.empty(sz.C_bytes // 4, dtype=torch.int32, device=self.device)
             self.S = torch.empty(sz.S_bytes, dtype=torch.uint8, device=self.device) if sz.S_bytes else None
-            self.W = torch.empty(sz.workspace_bytes, dtype=torch.uint8, device=self.device) if sz.workspace_bytes else None
+            self.W = torch.empty(sz.workspace_bytes, dtype=torch.uint8, device=self.device)
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             w = Weights((C.c_uint32 * 6)(*ct), (C.c_uint32 * 6)(*dir_mult), cost_one_log2, flags)
-            b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None,
-                        self.W.data_ptr() if self.W is not None else None)
+            b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None, self.W.data_ptr())
+            lim = Limits(max_footprint_radius, reach_levels)
             h = C.c_void_p()
-            rc = self._L.nhp_planner_create(C.byref(h), log2_n, log2_ntheta, float(R), C.byref(w), C.byref(b),
+            rc = self._L.nhp_planner_create(C.byref(h), log2_n, log2_ntheta, float(R), C.byref(w), C.byref(lim), C.byref(b),
                                             C.c_void_p(self.stream.cuda_stream))
         if rc:
             raise NhpError(rc, "planner_create")
@@ -206,7 +218,7 @@ class Planner:
         self._check(self._L.nhp_debug_soft_image(self._h, out.ctypes.data), "debug_soft_image")
         return out
 
-    def run_nturn(self, start, n_cycles=8):
+    def run_nturn(self, start, n_cycles=DEFAULT_CYCLES):
         self._check(self._L.nhp_run_nturn(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_cycles)), "run_nturn")
 
     def run_nturn_from(self, start, m0, n_cycles=8):
@@ -281,6 +293,18 @@ class Planner:
         self._check(self._L.nhp_debug_tables(self._h, *[t[k].ctypes.data for k in ("beta", "psi2", "B", "I", "J", "len_q")]),
                     "debug_tables")
         return t
+
+    def debug_footprint(self):
+        """E_Theta of the current footprint: (rad, covered uint8 [N_theta][2 rad + 1][2 rad + 1])."""
+        rad = C.c_int(0)
+        self._check(self._L.nhp_debug_footprint(self._h, C.byref(rad), None, 0), "debug_footprint")
+        side = 2 * rad.value + 1
+        cov = np.empty((self.nt, side, side), np.uint8)
+        self._check(self._L.nhp_debug_footprint(self._h, C.byref(rad), cov.ctypes.data, cov.nbytes), "debug_footprint")
+        return rad.value, cov
+
+    def prof_dropped(self):
+        return int(self._L.nhp_prof_dropped(self._h))
 
     def launch_count(self):
         return int(self._L.nhp_launch_count(self._h))

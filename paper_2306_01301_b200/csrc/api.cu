@@ -2,10 +2,13 @@
 // and kernel launches.  No planning arithmetic runs on the host after nhp_planner_create.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
 #include "nhp_internal.cuh"
+
+int set_kernel_attributes(nhp_planner *p);     // straight.cu: per-device function attributes, set at creation
 
 namespace {
 
@@ -119,55 +122,155 @@ int upload_tables(nhp_planner *p)
 
 bool in_grid(const nhp_planner *p, int i, int j, int t) { return i >= 0 && j >= 0 && t >= 0 && i < p->n && j < p->n && t < p->nt; }
 
+// Everything that scales with the grid or the limits lives in the caller's workspace (no allocation during
+// processing).  Offsets in bytes, each 256-byte aligned.
+struct WsLayout {
+    nhp_limits lim;                 // resolved
+    int side, sidew, cap_levels;
+    size_t cap_runs;
+    size_t soft_copies, reach, mask, E, runs, run_off, Hk, Mk, total;
+};
+
+WsLayout workspace_layout(int log2_n, int log2_nt, int flags, const nhp_limits *lim)
+{
+    WsLayout L{};
+    const size_t n = (size_t)1 << log2_n, nt = (size_t)1 << log2_nt, nr = n * n * nt;
+    int rmax = (lim && lim->max_footprint_radius > 0) ? lim->max_footprint_radius : 64;
+    if (rmax > (int)n / 2 - 1) rmax = (int)n / 2 - 1;
+    L.lim.max_footprint_radius = rmax;
+    L.lim.max_reach_levels = (lim && lim->max_reach_levels > 0) ? lim->max_reach_levels : 0;
+    L.side = 2 * rmax + 1; L.sidew = (L.side + 31) / 32;
+    L.cap_levels = 1;
+    while ((2 << (L.cap_levels - 1)) <= L.side) L.cap_levels++;            // floor(log2 side) + 1 levels of the sparse tables
+    L.cap_runs = nt * (size_t)L.side * 4 + 1;                              // <= 4 runs per footprint row on average
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    L.soft_copies = take((flags & NHP_FLAG_SOFT) ? 3 * nr : 0);            // S_left, S_right, S_line
+    L.reach = take(L.lim.max_reach_levels > 0 ? ((size_t)L.lim.max_reach_levels + 4) * (nr / 8) : 0);
+    L.mask = take((size_t)L.side * L.side);
+    L.E = take(sizeof(uint32_t) * nt * L.side * L.sidew);
+    L.runs = take(sizeof(int4) * L.cap_runs);
+    L.run_off = take(sizeof(int32_t) * (nt + 1));
+    L.Hk = take((n * n / 8) * L.cap_levels);
+    L.Mk = take((flags & NHP_FLAG_SOFT) ? n * n * L.cap_levels : 0);
+    L.total = off;
+    return L;
+}
+
+// Status words and the first NHP_PLAN_EAGER waypoints come back in one copy (they are contiguous on the device); the rest
+// of a longer plan, rarely, in a second one.  Step 8.
+int fetch_plan(nhp_planner *p, const int32_t *d_st)
+{
+    const size_t head = sizeof(int32_t) * NHP_STATUS_WORDS;
+    CU(cudaMemcpyAsync(p->h_status, d_st, head + sizeof(nhp_waypoint) * p->plan_eager, cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    const int n = p->h_status[2];
+    if (p->h_status[1] == NHP_OK && n > p->plan_eager) {
+        const size_t done = head + sizeof(nhp_waypoint) * p->plan_eager;
+        CU(cudaMemcpyAsync((uint8_t *)p->h_status + done, (const uint8_t *)d_st + done, sizeof(nhp_waypoint) * (size_t)(n - p->plan_eager),
+                           cudaMemcpyDeviceToHost, p->stream));
+        CU(cudaStreamSynchronize(p->stream));
+    }
+    return NHP_OK;
+}
+
 }  // namespace
+
+int set_kernel_attributes(nhp_planner *p);     // straight.cu: per-device function attributes, set at creation
+
+bool prof_grow(nhp_planner *p)
+{
+    const size_t pairs = p->ev.size() / 2;
+    if (pairs + PROF_GROW > (size_t)PROF_MAX_PAIRS) return false;
+    std::vector<cudaEvent_t> more(2 * PROF_GROW, nullptr);
+    for (auto &e : more)
+        if (cudaEventCreate(&e) != cudaSuccess) {
+            for (auto &f : more) if (f) cudaEventDestroy(f);
+            return false;
+        }
+    p->ev.insert(p->ev.end(), more.begin(), more.end());
+    p->ev_slot.resize(pairs + PROF_GROW, 0);
+    return true;
+}
 
 extern "C" {
 
-int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, nhp_sizes *out)
+int nhp_query_sizes(int log2_n, int log2_ntheta, int flags, const nhp_limits *lim, nhp_sizes *out)
 {
     if (!out) return NHP_E_ARG;
     if (log2_n < 5 || log2_n > 12 || log2_ntheta < 5 || log2_ntheta > 12) return NHP_E_NOT_POW2;
+    if (lim && (lim->max_footprint_radius < 0 || lim->max_reach_levels < 0 || lim->max_reach_levels > 254)) return NHP_E_ARG;
     const size_t nr = ((size_t)1 << (2 * log2_n)) << log2_ntheta;
     out->V_bytes = nr * 4;
     out->C_bytes = nr / 8;
     out->S_bytes = (flags & NHP_FLAG_SOFT) ? nr : 0;
-    out->workspace_bytes = (flags & NHP_FLAG_SOFT) ? 3 * nr : 0;        // curve-major copies of S (S_left, S_right, S_line)
+    out->workspace_bytes = workspace_layout(log2_n, log2_ntheta, flags, lim).total;
     return NHP_OK;
 }
 
 int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_cells, const nhp_weights *w,
-                       const nhp_buffers *dev, void *cuda_stream)
+                       const nhp_limits *lim, const nhp_buffers *dev, void *cuda_stream)
 {
     if (!out || !w || !dev) return NHP_E_ARG;
     *out = nullptr;
     if (log2_n < 5 || log2_n > 12 || log2_ntheta < 5 || log2_ntheta > 12) return NHP_E_NOT_POW2;
     if (!(R_cells >= 1.0) || w->cost_one_log2 < 0 || w->cost_one_log2 > 16) return NHP_E_ARG;
+    if (lim && (lim->max_footprint_radius < 0 || lim->max_reach_levels < 0 || lim->max_reach_levels > 254)) return NHP_E_ARG;
     if ((double)(1 << log2_ntheta) < 2.0 * kPi * R_cells) return NHP_E_ANGRES;
-    if (!dev->V || !dev->C || ((w->flags & NHP_FLAG_SOFT) && (!dev->S || !dev->workspace))) return NHP_E_BUFFER;
+    if (!dev->V || !dev->C || !dev->workspace || ((w->flags & NHP_FLAG_SOFT) && !dev->S)) return NHP_E_BUFFER;
     if (((uintptr_t)dev->V | (uintptr_t)dev->C | (uintptr_t)dev->S | (uintptr_t)dev->workspace) & 255) return NHP_E_BUFFER;
     nhp_planner *p = new (std::nothrow) nhp_planner();
     if (!p) return NHP_E_ARG;
     p->log2_n = log2_n; p->log2_nt = log2_ntheta; p->n = 1 << log2_n; p->nt = 1 << log2_ntheta;
     p->R = R_cells; p->w = *w; p->stream = (cudaStream_t)cuda_stream;
     p->V = (uint32_t *)dev->V; p->C = (uint32_t *)dev->C; p->S = (w->flags & NHP_FLAG_SOFT) ? (uint8_t *)dev->S : nullptr;
-    if (p->S) {
-        const size_t nr = (size_t)p->n * p->n * p->nt;
-        p->S_left = (uint8_t *)dev->workspace; p->S_right = p->S_left + nr; p->S_line = p->S_right + nr;
+    // the device that owns the caller's buffers is the handle's device
+    cudaPointerAttributes attr{};
+    if (cudaPointerGetAttributes(&attr, dev->V) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        delete p;
+        return NHP_E_BUFFER;
     }
+    p->device = attr.device;
+    DeviceGuard guard(p);
+    // carve the workspace
+    const WsLayout L = workspace_layout(log2_n, log2_ntheta, w->flags, lim);
+    p->lim = L.lim;
+    uint8_t *ws = (uint8_t *)dev->workspace;
+    const size_t nr = (size_t)p->n * p->n * p->nt;
+    if (p->S) { p->S_left = ws + L.soft_copies; p->S_right = p->S_left + nr; p->S_line = p->S_right + nr; }
+    if (L.lim.max_reach_levels > 0) {
+        const size_t W = nr / 32;
+        p->r_Lt = (uint32_t *)(ws + L.reach); p->r_Ct = p->r_Lt + W; p->r_Gt = p->r_Ct + W; p->r_levels = p->r_Gt + W;
+    }
+    p->d_mask = ws + L.mask; p->d_E = (uint32_t *)(ws + L.E);
+    p->d_runs = (int4 *)(ws + L.runs); p->d_run_off = (int32_t *)(ws + L.run_off);
+    p->d_Hk = (uint32_t *)(ws + L.Hk); p->d_Mk = p->S ? ws + L.Mk : nullptr;
+    p->cap_runs = L.cap_runs; p->cap_levels = L.cap_levels;
     int rc = build_tables(p);
     if (rc == NHP_OK) rc = upload_tables(p);
     const size_t npx = (size_t)p->n * p->n;
-    p->plan_cap = 4096;
+    p->plan_cap = NHP_PLAN_CAP;
+    if (const char *e = std::getenv("NHP_PLAN_EAGER")) {                 // test knob: exercise the second copy with short plans
+        const int v = std::atoi(e);
+        if (v >= 1 && v <= NHP_PLAN_CAP) p->plan_eager = v;
+    }
+    const size_t sp_bytes = sizeof(int32_t) * NHP_STATUS_WORDS + sizeof(nhp_waypoint) * p->plan_cap;      // status words + plan
     auto alloc = [&](void **ptr, size_t bytes) { if (rc == NHP_OK && cudaMalloc(ptr, bytes) != cudaSuccess) rc = NHP_E_CUDA; };
     alloc((void **)&p->d_hard, npx);
     alloc((void **)&p->d_soft, npx);
     if (w->flags & NHP_FLAG_SOFT) alloc((void **)&p->d_dtg, sizeof(int32_t) * npx);
-    alloc((void **)&p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS);
+    alloc((void **)&p->d_status, 2 * sp_bytes);
     alloc((void **)&p->d_goals, sizeof(int32_t) * 3 * NHP_MAX_GOALS);
-    alloc((void **)&p->d_plan, sizeof(nhp_waypoint) * p->plan_cap);
-    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sizeof(int32_t) * NHP_STATUS_WORDS) != cudaSuccess) rc = NHP_E_CUDA;
-    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_plan, sizeof(nhp_waypoint) * p->plan_cap) != cudaSuccess) rc = NHP_E_CUDA;
-    if (rc == NHP_OK && cudaMemsetAsync(p->d_status, 0, sizeof(int32_t) * NHP_STATUS_WORDS, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sp_bytes) != cudaSuccess) rc = NHP_E_CUDA;
+    if (rc == NHP_OK) {
+        p->d_plan = (nhp_waypoint *)(p->d_status + NHP_STATUS_WORDS);
+        p->d_rstatus = (int32_t *)((uint8_t *)p->d_status + sp_bytes);
+        p->d_rplan = (nhp_waypoint *)(p->d_rstatus + NHP_STATUS_WORDS);
+        p->h_plan = (nhp_waypoint *)(p->h_status + NHP_STATUS_WORDS);
+        if (cudaMemsetAsync(p->d_status, 0, 2 * sp_bytes, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
+    }
+    if (rc == NHP_OK) rc = set_kernel_attributes(p);
     if (rc != NHP_OK) { nhp_planner_destroy(p); return rc; }
     *out = p;
     return NHP_OK;
@@ -176,15 +279,14 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
 int nhp_planner_destroy(nhp_planner *p)
 {
     if (!p) return NHP_E_ARG;
-    cudaStreamSynchronize(p->stream);
-    cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
-    cudaFree(p->d_mask); cudaFree(p->d_E); cudaFree(p->d_hard); cudaFree(p->d_soft);
-    cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
-    cudaFree(p->d_status); cudaFree(p->d_plan); cudaFree(p->d_dtg); cudaFree(p->d_goals);
-    cudaFree(p->r_levels); cudaFree(p->r_Lt); cudaFree(p->r_Ct); cudaFree(p->r_Gt);
-    if (p->h_status) cudaFreeHost(p->h_status);
-    if (p->h_plan) cudaFreeHost(p->h_plan);
-    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    {
+        DeviceGuard guard(p);
+        cudaStreamSynchronize(p->stream);
+        cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
+        cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_status); cudaFree(p->d_dtg); cudaFree(p->d_goals);
+        if (p->h_status) cudaFreeHost(p->h_status);
+        for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    }
     delete p;
     return NHP_OK;
 }
@@ -199,22 +301,21 @@ int nhp_render_vehicle_footprint(nhp_planner *p, const uint8_t *mask_host, int m
     const double mv = std::fmax(std::fabs(-origin_v - 0.5), std::fabs((double)mh - 1.0 - origin_v + 0.5));
     const int rad = (int)std::ceil(std::hypot(mu, mv)) + 2;
     if (2 * rad >= p->n) return fail(p, NHP_E_ARG, "footprint does not fit the grid");
+    if (rad > p->lim.max_footprint_radius) return fail(p, NHP_E_BUFFER, "footprint radius exceeds nhp_limits.max_footprint_radius");
+    DeviceGuard guard(p);
     p->have_footprint = false;
-    CU(cudaStreamSynchronize(p->stream));
-    cudaFree(p->d_mask); cudaFree(p->d_E);
-    p->d_mask = nullptr; p->d_E = nullptr;
     p->rad = rad; p->side = 2 * rad + 1; p->sidew = (p->side + 31) / 32;
-    CU(cudaMalloc(&p->d_mask, (size_t)mw * mh));
-    CU(cudaMalloc(&p->d_E, sizeof(uint32_t) * (size_t)p->nt * p->side * p->sidew));
     CU(cudaMemcpyAsync(p->d_mask, mask_host, (size_t)mw * mh, cudaMemcpyHostToDevice, p->stream));
     const int64_t ouq = (int64_t)std::llround(origin_u * 32768.0), ovq = (int64_t)std::llround(origin_v * 32768.0);
     p->launches += launch_footprint_raster(p, mw, mh, ouq, ovq);
     CU(cudaGetLastError());
     CU(cudaStreamSynchronize(p->stream));            // mask_host may be freed by the caller after return
     const int frc = finish_footprint(p);
-    if (frc != NHP_OK) return fail(p, frc, "building the footprint run tables failed");
+    if (frc != NHP_OK) return fail(p, frc, frc == NHP_E_BUFFER ? "footprint mask breaks into more runs than the workspace holds" : "building the footprint run tables failed");
     p->have_footprint = true;
     p->have_render = false;
+    p->have_run = false;
+    p->r_n_levels = -1;
     return NHP_OK;
 }
 
@@ -233,6 +334,7 @@ int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *sof
     const bool want_soft = p->S != nullptr;
     if (want_soft && !soft) return fail(p, NHP_E_ARG, "NHP_FLAG_SOFT planner needs a soft image");
     if (!want_soft && soft) return fail(p, NHP_E_ARG, "soft image given but the planner has no soft volume");
+    DeviceGuard guard(p);
     const size_t npx = (size_t)p->n * p->n;
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     CU(cudaMemcpyAsync(p->d_hard, hard, npx, kind, p->stream));                       // step 3
@@ -240,7 +342,8 @@ int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *sof
     p->launches += launch_render(p, want_soft);                                       // step 4
     CU(cudaGetLastError());
     p->have_render = true;
-    p->have_run = false;
+    p->have_run = false;                  // both planners' results belong to the previous collision volume
+    p->r_n_levels = -1;
     return NHP_OK;
 }
 
@@ -250,6 +353,7 @@ int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, 
     if (!(k >= 0.0) || k > 64.0) return fail(p, NHP_E_ARG, "k outside [0, 64]");
     if (!p->have_footprint) return fail(p, NHP_E_STATE, "render_obstacles before render_vehicle_footprint");
     if (!p->S || !p->d_dtg) return fail(p, NHP_E_ARG, "the planner has no soft volume (NHP_FLAG_SOFT)");
+    DeviceGuard guard(p);
     const size_t npx = (size_t)p->n * p->n;
     const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     CU(cudaMemcpyAsync(p->d_hard, hard, npx, kind, p->stream));
@@ -258,6 +362,7 @@ int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, 
     CU(cudaGetLastError());
     p->have_render = true;
     p->have_run = false;
+    p->r_n_levels = -1;
     return NHP_OK;
 }
 
@@ -265,6 +370,7 @@ int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host)
 {
     if (!p || !soft_host) return fail(p, NHP_E_ARG, "NULL argument");
     if (!p->S || !p->have_render) return fail(p, NHP_E_STATE, "no soft image rendered yet");
+    DeviceGuard guard(p);
     CU(cudaMemcpyAsync(soft_host, p->d_soft, (size_t)p->n * p->n, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     return NHP_OK;
@@ -283,7 +389,8 @@ int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cy
         return fail(p, NHP_E_ARG, "a reverse maneuver cannot be in progress with NHP_FLAG_FORWARD_ONLY");
     if (!p->have_render) return fail(p, NHP_E_STATE, "run_nturn before render_obstacles");
     if (!in_grid(p, i, j, theta)) return fail(p, NHP_E_ARG, "start pose outside the grid");
-    if (n_cycles <= 0) n_cycles = 8;
+    if (n_cycles <= 0) n_cycles = NHP_DEFAULT_CYCLES;
+    DeviceGuard guard(p);
     p->start[0] = i; p->start[1] = j; p->start[2] = theta;
     p->start_m0 = m0;
     p->launches += launch_init_volume(p, i, j, theta);
@@ -300,11 +407,13 @@ int nhp_reach_run(nhp_planner *p, int i, int j, int theta, int n_levels)
     if (!p) return NHP_E_ARG;
     if (!p->have_render) return fail(p, NHP_E_STATE, "reach_run before render_obstacles");
     if (!in_grid(p, i, j, theta)) return fail(p, NHP_E_ARG, "start pose outside the grid");
-    if (n_levels <= 0) n_levels = 8;
+    if (n_levels <= 0) n_levels = NHP_DEFAULT_CYCLES;
     if (n_levels > 254) return fail(p, NHP_E_ARG, "more than 254 levels");
+    if (n_levels > p->lim.max_reach_levels) return fail(p, NHP_E_BUFFER, "n_levels exceeds nhp_limits.max_reach_levels of this planner");
+    DeviceGuard guard(p);
     int k = 0;
     const int rc = launch_reach_run(p, i, j, theta, n_levels, &k);
-    if (rc != NHP_OK) return fail(p, rc, "allocating the level volumes failed");
+    if (rc != NHP_OK) return fail(p, rc, "launching the level sweeps failed");
     p->launches += k;
     p->r_start[0] = i; p->r_start[1] = j; p->r_start[2] = theta;
     CU(cudaGetLastError());
@@ -325,6 +434,7 @@ int nhp_reach_count_volume(nhp_planner *p, uint8_t *K_dev)
     if (!p || !K_dev) return fail(p, NHP_E_ARG, "NULL argument");
     if (p->r_n_levels < 0) return fail(p, NHP_E_STATE, "reach_count_volume before reach_run");
     if ((uintptr_t)K_dev & 15) return fail(p, NHP_E_BUFFER, "K buffer must be 16-byte aligned");
+    DeviceGuard guard(p);
     p->launches += launch_reach_count(p, K_dev);
     CU(cudaGetLastError());
     return NHP_OK;
@@ -336,11 +446,10 @@ int nhp_reach_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypo
     if (p->r_n_levels < 0) return fail(p, NHP_E_STATE, "reach_extract_path before reach_run");
     if (!in_grid(p, gi, gj, gtheta)) return fail(p, NHP_E_ARG, "goal pose outside the grid");
     *count = 0; *n_maneuvers = -1;
+    DeviceGuard guard(p);
     p->launches += launch_reach_backtrack(p, gi, gj, gtheta);
     CU(cudaGetLastError());
-    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaStreamSynchronize(p->stream));
+    if (fetch_plan(p, p->d_rstatus) != NHP_OK) return NHP_E_CUDA;
     const int rc = p->h_status[1];
     if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
     if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "goal not reached within the levels of the last reach_run");
@@ -358,6 +467,7 @@ int nhp_run_more(nhp_planner *p, int n_cycles)
     if (!p) return NHP_E_ARG;
     if (!p->have_run) return fail(p, NHP_E_STATE, "run_more before run_nturn");
     if (n_cycles <= 0) return fail(p, NHP_E_ARG, "n_cycles must be positive");
+    DeviceGuard guard(p);
     if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
     p->launches += launch_cycles(p, n_cycles);
     CU(cudaGetLastError());
@@ -368,6 +478,7 @@ int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out)
 {
     if (!p || !dev_ptr_out) return NHP_E_ARG;
     if (!p->have_run) return fail(p, NHP_E_STATE, "cost_volume before run_nturn");
+    DeviceGuard guard(p);
     if (!p->canonical) { p->launches += launch_export_volume(p, true); p->canonical = true; }
     CU(cudaGetLastError());
     *dev_ptr_out = p->V;
@@ -377,6 +488,7 @@ int nhp_cost_volume(nhp_planner *p, const uint32_t **dev_ptr_out)
 int nhp_status(nhp_planner *p)
 {
     if (!p) return NHP_E_ARG;
+    DeviceGuard guard(p);
     CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
     CU(cudaStreamSynchronize(p->stream));
     if (p->have_run && p->h_status[0]) return fail(p, NHP_E_START_BLOCKED, "the start vertex collides");
@@ -389,12 +501,11 @@ int nhp_extract_path(nhp_planner *p, int gi, int gj, int gtheta, nhp_waypoint *o
     if (!p->have_run) return fail(p, NHP_E_STATE, "extract_path before run_nturn");
     if (!in_grid(p, gi, gj, gtheta)) return fail(p, NHP_E_ARG, "goal pose outside the grid");
     *count = 0; *cost = NHP_INF;
+    DeviceGuard guard(p);
     if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
     p->launches += launch_backtrack(p, gi, gj, gtheta);
     CU(cudaGetLastError());
-    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaStreamSynchronize(p->stream));                                             // step 8
+    if (fetch_plan(p, p->d_status) != NHP_OK) return NHP_E_CUDA;                      // step 8
     const int rc = p->h_status[1];
     if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
     if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "goal not reached");
@@ -418,14 +529,13 @@ int nhp_extract_path_goalset(nhp_planner *p, const int32_t *goals_host, int n_go
     for (int g = 0; g < n_goals; g++)
         if (!in_grid(p, goals_host[3 * g], goals_host[3 * g + 1], goals_host[3 * g + 2])) return fail(p, NHP_E_ARG, "goal pose outside the grid");
     *count = 0; *cost = NHP_INF;
+    DeviceGuard guard(p);
     if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
     CU(cudaMemcpyAsync(p->d_goals, goals_host, sizeof(int32_t) * 3 * n_goals, cudaMemcpyHostToDevice, p->stream));
     p->launches += launch_goal_search(p, n_goals, d, W, w);                           // step 6
     p->launches += launch_backtrack(p, -1, -1, -1);                                   // step 7
     CU(cudaGetLastError());
-    CU(cudaMemcpyAsync(p->h_status, p->d_status, sizeof(int32_t) * NHP_STATUS_WORDS, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaMemcpyAsync(p->h_plan, p->d_plan, sizeof(nhp_waypoint) * p->plan_cap, cudaMemcpyDeviceToHost, p->stream));
-    CU(cudaStreamSynchronize(p->stream));                                             // step 8
+    if (fetch_plan(p, p->d_status) != NHP_OK) return NHP_E_CUDA;                      // step 8
     const int rc = p->h_status[1];
     if (rc == NHP_E_START_BLOCKED) return fail(p, rc, "the start vertex collides");
     if (rc == NHP_E_GOAL_UNREACHED) return fail(p, rc, "no vertex of the goal set is reached");
@@ -473,14 +583,32 @@ int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t
 
 long long nhp_launch_count(const nhp_planner *p) { return p ? p->launches : 0; }
 
+long long nhp_prof_dropped(const nhp_planner *p) { return p ? p->ev_dropped : 0; }
+
+int nhp_debug_footprint(nhp_planner *p, int *radius, uint8_t *covered, size_t cap)
+{
+    if (!p || !radius) return fail(p, NHP_E_ARG, "NULL argument");
+    if (!p->have_footprint) return fail(p, NHP_E_STATE, "no footprint rendered yet");
+    *radius = p->rad;
+    if (!covered) return NHP_OK;
+    const size_t side = (size_t)p->side, need = (size_t)p->nt * side * side;
+    if (cap < need) return fail(p, NHP_E_BUFFER, "covered[] too small");
+    DeviceGuard guard(p);
+    std::vector<uint32_t> E((size_t)p->nt * side * p->sidew);
+    CU(cudaMemcpyAsync(E.data(), p->d_E, sizeof(uint32_t) * E.size(), cudaMemcpyDeviceToHost, p->stream));
+    CU(cudaStreamSynchronize(p->stream));
+    for (size_t t = 0; t < (size_t)p->nt; t++)
+        for (size_t r = 0; r < side; r++)
+            for (size_t c = 0; c < side; c++)
+                covered[(t * side + r) * side + c] = (E[(t * side + r) * p->sidew + (c >> 5)] >> (c & 31)) & 1u;
+    return NHP_OK;
+}
+
 int nhp_set_profiling(nhp_planner *p, int enable)
 {
     if (!p) return NHP_E_ARG;
-    if (enable && p->ev.empty()) {
-        p->ev.resize(2 * PROF_PAIRS);
-        p->ev_slot.assign(PROF_PAIRS, 0);
-        for (auto &e : p->ev) CU(cudaEventCreate(&e));
-    }
+    DeviceGuard guard(p);
+    if (enable && p->ev.empty() && !prof_grow(p)) return fail(p, NHP_E_CUDA, "creating the timing events failed");
     p->profiling = enable != 0;
     return NHP_OK;
 }
@@ -488,6 +616,7 @@ int nhp_set_profiling(nhp_planner *p, int enable)
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset)
 {
     if (!p) return NHP_E_ARG;
+    DeviceGuard guard(p);
     CU(cudaStreamSynchronize(p->stream));
     for (int k = 0; k < p->ev_used; k++) {
         float ms = 0.f;

@@ -76,6 +76,8 @@ struct nhp_planner {
     int log2_n = 0, log2_nt = 0, n = 0, nt = 0;
     double R = 0;
     nhp_weights w{};
+    nhp_limits lim{};              // resolved limits (defaults filled in)
+    int device = 0;                // ordinal of the device that owns the caller's buffers; current inside every call
     cudaStream_t stream = nullptr;
     uint32_t *V = nullptr, *C = nullptr;
     uint8_t *S = nullptr;
@@ -92,10 +94,12 @@ struct nhp_planner {
     int16_t *d_tlist = nullptr;    // [nt] slices with I = 0 first (n_xslices of them), then those with I = 1
     int n_xslices = 0;
     int32_t *d_rot = nullptr;      // [nt][4] cosq, sinq, 2*Psi0, 2*Psi1
-    // footprint
+    // footprint (all in the caller's workspace, sized for lim.max_footprint_radius)
     int rad = 0, side = 0, sidew = 0;
-    uint8_t *d_mask = nullptr;
+    uint8_t *d_mask = nullptr;     // [(2 rmax + 1)^2]
     uint32_t *d_E = nullptr;       // [nt][side][sidew] bitmap of covered pixel offsets, bit (da + rad)
+    size_t cap_runs = 0;           // capacity of d_runs, entries
+    int cap_levels = 1;            // capacity of d_Hk / d_Mk, levels
     bool have_footprint = false;
     // images
     uint8_t *d_hard = nullptr, *d_soft = nullptr;
@@ -110,33 +114,51 @@ struct nhp_planner {
     int start[3] = {0, 0, 0};
     // reachability (bit-vector) planner, reach.cu: level volumes and the transposed working volumes (allocated at the first
     // nhp_reach_run), number of levels of the last run, its start
-    uint32_t *r_levels = nullptr, *r_Lt = nullptr, *r_Ct = nullptr, *r_Gt = nullptr;
-    int r_cap_levels = 0, r_n_levels = -1, r_start[3] = {0, 0, 0};
+    uint32_t *r_levels = nullptr, *r_Lt = nullptr, *r_Ct = nullptr, *r_Gt = nullptr;   // in the caller's workspace
+    int r_n_levels = -1, r_start[3] = {0, 0, 0};
     int start_m0 = -1;             // maneuver in progress at the start (nhp_run_nturn_from), -1 = none
     // plan extraction
-    int32_t *d_status = nullptr;   // [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search: i, j, theta, goal
-                                   // index, [8..9] its score, [10] found; NHP_STATUS_WORDS words
+    int32_t *d_status = nullptr;   // N-turn planner: [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search:
+                                   // i, j, theta, goal index, [8..9] its score, [10] found; NHP_STATUS_WORDS words.  The plan
+                                   // follows directly (d_plan = d_status + NHP_STATUS_WORDS): one copy brings both back
+    int32_t *d_rstatus = nullptr;  // reachability planner: its own [0] start blocked, [1] rc, [2] count, [3] maneuvers, then its plan
     int32_t *d_goals = nullptr;    // [NHP_MAX_GOALS][3] ideal goals of nhp_extract_path_goalset
-    nhp_waypoint *d_plan = nullptr;
-    int plan_cap = 0;
-    int32_t *h_status = nullptr;   // pinned
+    nhp_waypoint *d_plan = nullptr, *d_rplan = nullptr;
+    int plan_cap = 0, plan_eager = 128;    // waypoints brought back together with the status words (NHP_PLAN_EAGER)
+    int32_t *h_status = nullptr;   // pinned: NHP_STATUS_WORDS words, then plan_cap waypoints
     nhp_waypoint *h_plan = nullptr;
     std::string err = "ok";
     long long launches = 0;
     // per-kernel timing (nhp_set_profiling): event pairs on the launching stream, drained at sync points
     bool profiling = false;
-    std::vector<cudaEvent_t> ev;   // 2 * PROF_PAIRS events, created on first enable
+    std::vector<cudaEvent_t> ev;   // 2 events per pair; the pool grows by PROF_GROW pairs when it runs out, up to PROF_MAX_PAIRS
     std::vector<int> ev_slot;      // slot of each used pair
     int ev_used = 0;
+    long long ev_dropped = 0;      // launches that ran untimed because the pool was at its maximum
     double k_ms[NHP_KERNEL_SLOTS] = {0};
     long long k_launches[NHP_KERNEL_SLOTS] = {0};
 
     DevTables tables() const { return DevTables{d_beta, d_B, d_lenq, d_IJ}; }
 };
 
-constexpr int PROF_PAIRS = 1024;
+constexpr int PROF_GROW = 1024, PROF_MAX_PAIRS = 65536;
 constexpr int NHP_STATUS_WORDS = 16;
 constexpr int NHP_MAX_GOALS = 256;
+constexpr int NHP_PLAN_CAP = 4096;         // waypoints of the internal plan buffers
+
+bool prof_grow(nhp_planner *p);            // api.cu: add PROF_GROW event pairs; false at the maximum or on a CUDA error
+
+// Makes the handle's device current for the duration of an ABI call (the caller may have another one current).
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const nhp_planner *p)
+    {
+        if (!p) return;
+        int cur = -1;
+        if (cudaGetDevice(&cur) == cudaSuccess && cur != p->device) { prev = cur; cudaSetDevice(p->device); }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 // Bracket one kernel launch (or one group of launches) with an event pair when profiling is on.
 struct ProfScope {
@@ -144,7 +166,8 @@ struct ProfScope {
     int pair;
     ProfScope(nhp_planner *p_, int slot) : p(p_), pair(-1)
     {
-        if (!p->profiling || p->ev_used >= PROF_PAIRS) return;
+        if (!p->profiling) return;
+        if (2 * (size_t)p->ev_used >= p->ev.size() && !prof_grow(p)) { p->ev_dropped++; return; }
         pair = p->ev_used++;
         p->ev_slot[pair] = slot;
         cudaEventRecord(p->ev[2 * pair], p->stream);
@@ -157,7 +180,7 @@ struct ProfScope {
 
 // ---- kernel launchers (each returns the number of kernels it launched) ---------------------------
 int launch_footprint_raster(nhp_planner *p, int mw, int mh, int64_t ouq, int64_t ovq);
-int finish_footprint(nhp_planner *p);                 // host: run lists + table allocation; returns an NHP_ code
+int finish_footprint(nhp_planner *p);                 // host: run lists into the workspace tables; returns an NHP_ code
 int launch_render(nhp_planner *p, bool soft);
 int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);

@@ -314,14 +314,7 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
 {
     const int n = p->n, nt = p->nt, nw = n / 32;
     const size_t W = (size_t)n * n * nt / 32;
-    if (p->r_cap_levels < n_levels + 1) {                       // (re)allocate: the only allocation outside nhp_planner_create
-        cudaStreamSynchronize(p->stream);
-        cudaFree(p->r_levels); cudaFree(p->r_Lt); cudaFree(p->r_Ct); cudaFree(p->r_Gt);
-        p->r_levels = p->r_Lt = p->r_Ct = p->r_Gt = nullptr; p->r_cap_levels = 0;
-        if (cudaMalloc(&p->r_levels, sizeof(uint32_t) * W * (n_levels + 1)) != cudaSuccess || cudaMalloc(&p->r_Lt, sizeof(uint32_t) * W) != cudaSuccess ||
-            cudaMalloc(&p->r_Ct, sizeof(uint32_t) * W) != cudaSuccess || cudaMalloc(&p->r_Gt, sizeof(uint32_t) * W) != cudaSuccess) return NHP_E_CUDA;
-        p->r_cap_levels = n_levels + 1;
-    }
+    if (!p->r_levels || n_levels > p->lim.max_reach_levels) return NHP_E_BUFFER;      // volumes are carved from the workspace at creation
     const bool fwd_only = p->w.flags & NHP_FLAG_FORWARD_ONLY;
     const int nx = p->n_xslices, ny = nt - nx;
     const int trows = n / 32 < 8 ? n / 32 : 8;                  // 32 x 32 blocks per CTA of the transposition
@@ -339,7 +332,7 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
     geom(nt, PLn, tblk2, tw, t2smem, nt);
     geom(n, PLr, rblk2, rw, r2smem, 0);
     int k = 0;
-    reach_init_kernel<<<(unsigned)((W + 255) / 256), 256, 0, p->stream>>>(p->r_levels, p->C, W, ((size_t)st * n + sj) * n + si, p->d_status);
+    reach_init_kernel<<<(unsigned)((W + 255) / 256), 256, 0, p->stream>>>(p->r_levels, p->C, W, ((size_t)st * n + sj) * n + si, p->d_rstatus);
     if (nx > 0) reach_transpose_kernel<false><<<tgrid, tblk, 0, p->stream>>>(p->r_Ct, p->C, p->d_tlist, p->log2_n);
     k += 2;
     for (int m = 0; m < n_levels; m++) {
@@ -420,6 +413,6 @@ int launch_reach_backtrack(nhp_planner *p, int gi, int gj, int gt)
     P.gi = gi; P.gj = gj; P.gt = gt; P.cap = p->plan_cap;
     P.level_words = (size_t)p->n * p->n * p->nt / 32;
     ProfScope prof(p, 9);
-    reach_backtrack_kernel<<<1, 192, 0, p->stream>>>(p->r_levels, p->C, p->tables(), P, p->d_plan, p->d_status);
+    reach_backtrack_kernel<<<1, 192, 0, p->stream>>>(p->r_levels, p->C, p->tables(), P, p->d_rplan, p->d_rstatus);
     return 1;
 }

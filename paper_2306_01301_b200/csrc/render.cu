@@ -86,15 +86,10 @@ int finish_footprint(nhp_planner *p)
     }
     off[nt] = (int32_t)runs.size();
     if (runs.empty()) runs.push_back(make_int4(0, 0, 0, 0));
-    cudaFree(p->d_runs); cudaFree(p->d_run_off); cudaFree(p->d_Hk); cudaFree(p->d_Mk);
-    p->d_runs = nullptr; p->d_run_off = nullptr; p->d_Hk = nullptr; p->d_Mk = nullptr;
+    // the tables live in the caller's workspace, sized at creation for nhp_limits.max_footprint_radius
+    if (runs.size() > p->cap_runs || maxk + 1 > p->cap_levels) return NHP_E_BUFFER;
     p->n_levels = maxk + 1;
     p->max_runs = maxruns;
-    const size_t npx = (size_t)p->n * p->n;
-    if (cudaMalloc(&p->d_runs, sizeof(int4) * runs.size()) != cudaSuccess) return NHP_E_CUDA;
-    if (cudaMalloc(&p->d_run_off, sizeof(int32_t) * (nt + 1)) != cudaSuccess) return NHP_E_CUDA;
-    if (cudaMalloc(&p->d_Hk, (npx / 8) * p->n_levels) != cudaSuccess) return NHP_E_CUDA;
-    if (p->S && cudaMalloc(&p->d_Mk, npx * p->n_levels) != cudaSuccess) return NHP_E_CUDA;
     if (cudaMemcpyAsync(p->d_runs, runs.data(), sizeof(int4) * runs.size(), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) return NHP_E_CUDA;
     if (cudaMemcpyAsync(p->d_run_off, off.data(), sizeof(int32_t) * (nt + 1), cudaMemcpyHostToDevice, p->stream) != cudaSuccess) return NHP_E_CUDA;
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) return NHP_E_CUDA;

@@ -65,13 +65,14 @@ int launch_soft_layouts(nhp_planner *p)
 {
     const int n = p->n, nt = p->nt;
     const size_t smem = (size_t)32 * (nt + 16);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(soft_turn_layout_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * (4096 + 16));
-        attr_set = true;
-    }
     soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
     soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
     soft_line_layout_kernel<<<dim3(n / 32, n / 32, nt), dim3(32, 8), 0, p->stream>>>(p->S_line, p->S, p->d_B, p->d_IJ, p->log2_n);
     return 3;
+}
+
+// function attributes are per device: set for the handle's device at creation (nhp_planner_create)
+int set_softlayout_attributes()
+{
+    return cudaFuncSetAttribute(soft_turn_layout_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * (4096 + 16)) == cudaSuccess ? NHP_OK : NHP_E_CUDA;
 }

@@ -202,7 +202,7 @@ __device__ __forceinline__ void xr_stage_store(const uint32_t *sp, unsigned long
 
 template <bool SOFT>
 __device__ __forceinline__ void xr_band_sweep(uint32_t *__restrict__ Vslice, const uint8_t *__restrict__ Sl, const int16_t *__restrict__ Bt,
-                                              uint32_t *buf, int X0, int lane, int log2_n, uint32_t w, uint32_t ct, bool up)
+                                              uint32_t *buf, int X0, int lane, int log2_n, uint32_t w, uint32_t ct, bool up, int fixed)
 {
     constexpr int SW = XR_TILE_WORDS + (SOFT ? 256 : 0);
     const int NT = 1 << (log2_n - 5);
@@ -235,9 +235,10 @@ __device__ __forceinline__ void xr_band_sweep(uint32_t *__restrict__ Vslice, con
             s0 = sl[lane]; s1 = sl[32 + lane];
         }
         uint32_t cm = 0;
-        if (tile_is_idle(u, t)) { }
+        if (!fixed && tile_is_idle(u, t)) { }
         else if (up) RelaxLoop<true, SOFT>::run(u, t, wp, w, ct, s0, s1, cm);
         else RelaxLoop<false, SOFT>::run(u, t, wp, w, ct, s0, s1, cm);
+        if (fixed) cm = 0xffffffffu;                       // NHP_FLAG_FIXED_WORK: every vertex goes back
         const uint32_t lines = __ballot_sync(0xffffffffu, cm != 0u);
         if (lines) {
             xr_scatter(u, row, offs4, cm);
@@ -253,7 +254,7 @@ template <bool SOFT>
 __global__ void __launch_bounds__(128) straight_xrows_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
                                                              const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
                                                              const int16_t *__restrict__ tlist,
-                                                             const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward)
+                                                             const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward, int fixed)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     constexpr int SW = XR_TILE_WORDS + (SOFT ? 256 : 0);
@@ -267,7 +268,7 @@ __global__ void __launch_bounds__(128) straight_xrows_kernel(uint32_t *__restric
     const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) : nullptr;
     uint32_t *buf = smem + warp * (XR_NBUF * SW);
     const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
-    xr_band_sweep<SOFT>(Vt, Sl, Bt, buf, X0, lane, log2_n, w, ct, up);
+    xr_band_sweep<SOFT>(Vt, Sl, Bt, buf, X0, lane, log2_n, w, ct, up, fixed);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -283,7 +284,7 @@ template <bool SOFT>
 __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
                                                             const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
                                                             const int16_t *__restrict__ tlist,
-                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward)
+                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward, int fixed)
 {
     const int n = 1 << log2_n, mx = n - 1, t = tlist[blockIdx.y];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -313,9 +314,10 @@ __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restr
         uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
         if (SOFT) { s0 = ld_nc16(Sl + 32 * T); s1 = ld_nc16(Sl + 32 * T + 16); }
         uint32_t cm = 0;
-        if (tile_is_idle(u, tv)) { }
+        if (!fixed && tile_is_idle(u, tv)) { }
         else if (up) RelaxLoop<true, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
         else RelaxLoop<false, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
+        if (fixed) cm = 0xffffffffu;                       // NHP_FLAG_FIXED_WORK: every vertex goes back
         if (__any_sync(0xffffffffu, cm != 0u)) {
 #pragma unroll
             for (int k = 0; k < 32; k++) {
@@ -339,23 +341,30 @@ int launch_straight_tile(nhp_planner *p, int m)
     const int bands = n / 32, warps = bands < 4 ? bands : 4, xwarps = bands < XR_WARPS_V ? bands : XR_WARPS_V;
     const int sw = XR_TILE_WORDS + (soft ? 256 : 0);
     const size_t smem = sizeof(uint32_t) * (size_t)xwarps * XR_NBUF * sw;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(straight_xrows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * XR_NBUF * XR_TILE_WORDS * 4);
-        cudaFuncSetAttribute(straight_xrows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * XR_NBUF * (XR_TILE_WORDS + 256) * 4);
-        attr_set = true;
-    }
     ProfScope prof(p, m);
     const uint32_t *lenq = p->d_lenq + (size_t)m * nt;
     const int nx = p->n_xslices, ny = nt - nx;
     const dim3 gx(bands / xwarps, nx), gy(bands / warps, ny);
     const int fwd = (m == M_SF);
+    const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : 0;
     if (soft) {
-        straight_xrows_kernel<true><<<gx, xwarps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd);
-        straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd);
+        straight_xrows_kernel<true><<<gx, xwarps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
     } else {
-        straight_xrows_kernel<false><<<gx, xwarps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd);
-        straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd);
+        straight_xrows_kernel<false><<<gx, xwarps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
     }
     return 2;
+}
+
+int set_softlayout_attributes();               // softlayout.cu
+
+// Function attributes are per device: set for the handle's device (current here) at creation.
+int set_kernel_attributes(nhp_planner *p)
+{
+    (void)p;
+    if (cudaFuncSetAttribute(straight_xrows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * XR_NBUF * XR_TILE_WORDS * 4) != cudaSuccess ||
+        cudaFuncSetAttribute(straight_xrows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * XR_NBUF * (XR_TILE_WORDS + 256) * 4) != cudaSuccess)
+        return NHP_E_CUDA;
+    return set_softlayout_attributes();
 }

@@ -400,7 +400,7 @@ __device__ __forceinline__ void tile_rows_store(const uint32_t (&col)[L], uint32
 template <int L, int NPASS, bool UP0, bool SOFT>
 __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Scurve,
                                                           const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb,
-                                                          TurnPass pa, TurnPass pb, uint32_t one)
+                                                          TurnPass pa, TurnPass pb, uint32_t one, int fixed)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
@@ -433,12 +433,14 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     unsigned long long before = 0, after = 0;
 #pragma unroll
     for (int k = 0; k < L; k++) checksum_add(before, col[k], one);
-    const bool all_blocked = __all_sync(0xffffffffu, before == 0ull);
+    // `fixed` (NHP_FLAG_FIXED_WORK) switches the three short cuts off and stores every row: the same instructions and
+    // bytes whatever the volume holds
+    const bool all_blocked = !fixed && __all_sync(0xffffffffu, before == 0ull);
     // (soft kernels keep one chain variant: a second copy of their loops costs registers they do not have)
-    const bool none_blocked = !SOFT && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
+    const bool none_blocked = !SOFT && !fixed && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
     // "no finite value in this warp yet": min over (v - 1) with wrap-around (blocked 0 -> 2^32 - 1, unreached -> 2^30)
     bool no_finite = false;
-    if (!SOFT) {
+    if (!SOFT && !fixed) {
         uint32_t lowest = 0xffffffffu;
 #pragma unroll
         for (int k = 0; k < L; k++) lowest = __viaddmin_u32(col[k], 0xffffffffu, lowest);
@@ -457,7 +459,7 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
             for (int k = 0; k < L; k++) checksum_add(after, col[k], one);
         }
     }
-    if (after != before) {
+    if (after != before || fixed) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills
         if (!wraps) tile_rows_store<L, false>(col, V, so + row0, lane, (uint32_t)mx);
@@ -489,10 +491,11 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     };
     const TurnPass pa = pass(ma), pb = pass(mb);
     const uint8_t *Sc = left ? p->S_left : p->S_right;
+    const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : 0;
     const dim3 grid(n / 32, n), block(32 * S);
     const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 4 * (size_t)S * 32;
     ProfScope prof(p, mb >= 0 ? 11 : ma);
-#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u)
+#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u, fixed)
 #define NHP_TT2(NP, UP) do { if (soft) NHP_TT(NP, UP, true); else NHP_TT(NP, UP, false); } while (0)
     if (mb >= 0) { if (up) NHP_TT2(2, true); else NHP_TT2(2, false); }
     else { if (up) NHP_TT2(1, true); else NHP_TT2(1, false); }

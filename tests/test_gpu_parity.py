@@ -40,7 +40,7 @@ def small_scenes():
     ]
 
 
-@pytest.mark.parametrize("flags", [0, 4])
+@pytest.mark.parametrize("flags", [0, 4, 8])     # tile kernels, thread-per-curve kernels, NHP_FLAG_FIXED_WORK (short cuts off)
 def test_tables_render_sweeps_and_plans_match_the_oracle(mods, flags):
     oracle, nhp = mods
     for sc in small_scenes():
@@ -154,7 +154,8 @@ def test_reachability_planner_of_appendix_c(mods):
         o, fp = oracle_for(oracle, sc)
         Cv, _ = o.render(fp, sc.hard, None, method="runs")
         K = o.reach_run(Cv, sc.start, n_levels)
-        p = nhp.Planner.from_scene(sc) if sc.soft is None else nhp.Planner(sc.log2_n, sc.log2_nt, sc.R, sc.ct, flags=sc.flags & 1)
+        p = (nhp.Planner.from_scene(sc, reach_levels=n_levels) if sc.soft is None else
+             nhp.Planner(sc.log2_n, sc.log2_nt, sc.R, sc.ct, flags=sc.flags & 1, reach_levels=n_levels))
         if sc.soft is not None:
             p.render_vehicle_footprint(sc.mask, sc.ou, sc.ov)
         p.render_obstacles(sc.hard)
@@ -170,9 +171,12 @@ def test_reachability_planner_of_appendix_c(mods):
             with pytest.raises(nhp.NhpError) as e:
                 p.reach_extract_path((int(ij[0]), int(jj[0]), int(tj[0])))
             assert e.value.code == -5
-        # a second, shorter run reuses the buffers
+        # a second, shorter run reuses the buffers; more levels than the planner was created for are refused
         p.reach_run(sc.start, 2)
         assert (p.reach_count_numpy() == o.reach_run(Cv, sc.start, 2)).all()
+        with pytest.raises(nhp.NhpError) as e:
+            p.reach_run(sc.start, n_levels + 1)
+        assert e.value.code == -6
         p.close()
 
 
@@ -184,7 +188,7 @@ def test_reachability_planner_config3_maze_512(mods):
     o, fp = oracle_for(oracle, sc)
     Cv, _ = o.render(fp, sc.hard, None, method="runs")
     K = o.reach_run(Cv, sc.start, sc.n_cycles)
-    p = nhp.Planner.from_scene(sc)
+    p = nhp.Planner.from_scene(sc, reach_levels=sc.n_cycles)
     p.render_obstacles(sc.hard)
     p.reach_run(sc.start, sc.n_cycles)
     got = p.reach_count_numpy()
@@ -193,6 +197,146 @@ def test_reachability_planner_config3_maze_512(mods):
     for t, j, i in far[:: max(1, len(far) // 8)][:8]:
         goal = (int(i), int(j), int(t))
         assert p.reach_extract_path(goal) == o.reach_backtrack(K, Cv, sc.start, goal), goal
+    p.close()
+
+
+def test_footprint_elements_match_the_oracle(mods):
+    """The structuring elements E_Theta (DESIGN R15) through nhp_debug_footprint against the oracle's orc_footprint_offsets,
+    at every Theta: box vehicles, a mask with a hole and a notch, a fractional origin."""
+    oracle, nhp = mods
+    holed = np.ones((5, 9), np.uint8)
+    holed[2, 3:6] = 0
+    holed[0, 0] = 0
+    cases = [(5, 5, 4, np.ones((2, 4), np.uint8), 0.3, 0.5), (6, 6, 8, np.ones((3, 7), np.uint8), 0.9, 1.0), (5, 7, 4, holed, 2.25, 1.75),
+             (7, 6, 9, np.ones((9, 20), np.uint8), 3.5, 4.0)]
+    for log2_n, log2_nt, R, mask, ou, ov in cases:
+        o = oracle.Oracle(log2_n, log2_nt, R, (1024,) * 6)
+        fp = oracle.Footprint(mask, ou, ov)
+        p = nhp.Planner(log2_n, log2_nt, R, (1024,) * 6)
+        p.render_vehicle_footprint(mask, ou, ov)
+        rad, cov = p.debug_footprint()
+        assert rad == fp.radius()
+        for t in range(o.nt):
+            da, db = o.footprint_offsets(fp, t)
+            want = np.zeros((2 * rad + 1, 2 * rad + 1), np.uint8)
+            want[db + rad, da + rad] = 1
+            assert (cov[t] == want).all(), (mask.shape, t)
+        p.close()
+    # a footprint beyond the limit the planner was created for is refused, and so is one that does not fit the grid
+    p = nhp.Planner(7, 6, 9, (1024,) * 6, max_footprint_radius=8)
+    with pytest.raises(nhp.NhpError) as e:
+        p.render_vehicle_footprint(np.ones((9, 20), np.uint8), 3.5, 4.0)
+    assert e.value.code == -6
+    p.set_box(4, 1, 1)
+    p.close()
+
+
+def test_the_two_planners_keep_their_state_apart(mods):
+    """One handle runs the N-turn planner and the reachability planner in any order: a blocked start of one must not leak
+    into the other, and a new rendering invalidates the results of both."""
+    oracle, nhp = mods
+    sc = scenes.random_scene(6, 5, 5, 71, n_rects=8)
+    o, fp = oracle_for(oracle, sc)
+    Cv, _ = o.render(fp, sc.hard, None, method="brute")
+    blocked = (0, 7, 3)                                               # wall cell
+    p = nhp.Planner.from_scene(sc, reach_levels=6)
+    p.render_obstacles(sc.hard)
+    V = o.run(Cv, None, sc.start, 3)
+    K = o.reach_run(Cv, sc.start, 6)
+    tj, jj, ij = np.nonzero((V != INF) & (K != 255))
+    goal = (int(ij[len(ij) // 2]), int(jj[len(ij) // 2]), int(tj[len(ij) // 2]))
+    # N-turn run from a good start, then a reachability run from a blocked one
+    p.run_nturn(sc.start, 3)
+    p.reach_run(blocked, 6)
+    with pytest.raises(nhp.NhpError) as e:
+        p.reach_extract_path(goal)
+    assert e.value.code == -4
+    p.status()                                                        # the N-turn run is not affected
+    assert p.extract_path(goal) == o.backtrack(V, Cv, None, sc.start, goal)
+    # and the other way round
+    p.reach_run(sc.start, 6)
+    p.run_nturn(blocked, 3)
+    with pytest.raises(nhp.NhpError) as e:
+        p.extract_path(goal)
+    assert e.value.code == -4
+    assert p.reach_extract_path(goal) == o.reach_backtrack(K, Cv, sc.start, goal)
+    # a new rendering: neither planner may back-track its old volumes against the new collision volume
+    p.run_nturn(sc.start, 3)
+    p.render_obstacles(np.zeros_like(sc.hard))
+    for call in (lambda: p.extract_path(goal), lambda: p.reach_extract_path(goal), lambda: p.reach_count_numpy(), lambda: p.cost_volume()):
+        with pytest.raises(nhp.NhpError) as e:
+            call()
+        assert e.value.code == -8
+    p.render_vehicle_footprint(sc.mask, sc.ou, sc.ov)                # a new footprint invalidates the rendering as well
+    with pytest.raises(nhp.NhpError) as e:
+        p.run_nturn(sc.start, 1)
+    assert e.value.code == -8
+    p.close()
+
+
+def test_no_device_allocation_after_create(mods):
+    """PAPER.md:565 "no memory allocation takes place during processing": after nhp_planner_create (and one warm-up plan,
+    which loads the kernels' code) a footprint change, rendering, both planners and path extraction leave the device's free
+    memory where it was."""
+    oracle, nhp = mods
+    import torch
+    sc = scenes.random_scene(7, 6, 9, 72, vehicle=(9, 4), n_rects=20, soft=True, reverse_mult=300, n_cycles=2)
+    p = nhp.Planner.from_scene(sc, reach_levels=5)
+    K = torch.empty(p.shape, dtype=torch.uint8, device=p.device)
+
+    def everything():
+        p.render_vehicle_footprint(sc.mask, sc.ou, sc.ov)
+        p.render_obstacles(sc.hard, sc.soft)
+        p.render_obstacles_dt(sc.hard, 4.0)
+        p.run_nturn(sc.start, 2)
+        p.run_nturn_from(sc.start, 1, 1)
+        p.run_more(1)
+        p.cost_volume()
+        p.status()
+        try:
+            p.extract_path(sc.goal)
+            p.extract_path_goalset([sc.goal], 3, 10, 10)
+        except nhp.NhpError as e:
+            assert e.code == -5
+        p.reach_run(sc.start, 5)
+        p._check(p._L.nhp_reach_count_volume(p._h, K.data_ptr()), "reach_count_volume")
+        try:
+            p.reach_extract_path(sc.goal)
+        except nhp.NhpError as e:
+            assert e.code == -5
+        torch.cuda.synchronize()
+
+    everything()
+    free0, _ = torch.cuda.mem_get_info()
+    everything()
+    everything()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 == free0, (free0, free1)
+    p.close()
+
+
+def test_default_cycles_and_long_plans(mods, monkeypatch):
+    """n_cycles <= 0 selects the paper's default of 8 cycles; a plan longer than the waypoints that travel with
+    the status words comes back complete (second copy)."""
+    oracle, nhp = mods
+    sc = scenes.random_scene(6, 6, 8, 73, n_rects=14)
+    o, fp = oracle_for(oracle, sc)
+    Cv, _ = o.render(fp, sc.hard, None, method="brute")
+    V = o.run(Cv, None, sc.start, 8)
+    monkeypatch.setenv("NHP_PLAN_EAGER", "2")
+    p = nhp.Planner.from_scene(sc)
+    p.render_obstacles(sc.hard)
+    p.run_nturn(sc.start, 0)
+    assert (p.cost_volume_numpy() == V).all()
+    tj, jj, ij = np.nonzero(V != INF)
+    order = np.argsort(V[tj, jj, ij])[::-1][:20]                     # the most expensive goals have the longest plans
+    longest = 0
+    for k in order:
+        goal = (int(ij[k]), int(jj[k]), int(tj[k]))
+        want = o.backtrack(V, Cv, None, sc.start, goal)
+        assert p.extract_path(goal) == want
+        longest = max(longest, len(want[0]))
+    assert longest > 3
     p.close()
 
 
