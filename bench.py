@@ -26,7 +26,8 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-METRIC = "pose_updates_per_sec (N-turn planner, whole plan: render + N_T maneuver cycles + back-track)"
+METRIC = "pose_updates_per_sec (N-turn planner, whole plan: render + N_T maneuver cycles + back-track)"   # ours; the reference arm
+# times maneuver sweeps of the oracle over the same volume (its `sample` says which) and reports them in the same unit
 UNIT = "Gpose-updates/s"
 FALLBACK_HBM_GBS = 6650.0            # /opt/skills/guides/B200_PROFILING.md fallback
 ALG_BYTES_HARD, ALG_BYTES_SOFT = 8.125, 9.125     # read V 4 + write V 4 + 1 collision bit [+ 1 soft byte]
@@ -44,6 +45,8 @@ def parse_args():
     ap.add_argument("--simple-kernels", action="store_true", help="thread-per-curve bring-up kernels (A/B)")
     ap.add_argument("--reach", action="store_true",
                     help="time the reachability (bit-vector) planner of appendix C instead: render + N_T levels + back-track")
+    ap.add_argument("--fixed-work", action="store_true", help="NHP_FLAG_FIXED_WORK: data-dependent short cuts off (PAPER.md:565)")
+    ap.add_argument("--no-extra", action="store_true", help="skip the fixed-work pass and the configs 4 / 5 side runs")
     ap.add_argument("--dt-on-device", action="store_true",
                     help="soft configs: distance transform + soft image on the GPU (nhp_render_obstacles_dt) instead of the harness image")
     return ap.parse_args()
@@ -134,7 +137,152 @@ def pick_goal(p, sc, torch):
     return tuple(cands[best]) if vals[best] != 0xFFFFFFFF else tuple(sc.start)
 
 
+SWEEP_SLOTS = ("turn_pair", "LF", "RB", "RF", "LB", "straight_xrows", "straight_rows")
+
+
+class PlanBench:
+    """One planner on one scene: warm-up, goal choice, and timed passes of `step` = render + N_T cycles + back-track."""
+
+    def __init__(self, nhp, torch, replicas, sc, n_cycles, dev, flags=0, reach=False, dt_on_device=False):
+        self.nhp, self.torch, self.replicas, self.sc, self.n_cycles, self.dev = nhp, torch, replicas, sc, n_cycles, dev
+        self.reach, self.dt_dev = reach, dt_on_device and sc.soft is not None
+        self.p = nhp.Planner.from_scene(sc, flags=flags, device=dev, reach_levels=n_cycles if reach else 0)
+        self.hard_d = torch.from_numpy(sc.hard).to(dev)
+        self.soft_d = torch.from_numpy(sc.soft).to(dev) if sc.soft is not None else None
+        self.hard_h = torch.from_numpy(sc.hard).pin_memory()
+        self.soft_h = torch.from_numpy(sc.soft).pin_memory() if sc.soft is not None else None
+        self.goal, self.plan = tuple(sc.goal), None
+        self.n_r = sc.n * sc.n * sc.nt
+        self.updates_per_plan = 6 * n_cycles * self.n_r
+        I = self.p.debug_tables()["I"]
+        self.nx = int((I == 0).sum())                                   # slices swept by the x-rows kernel (eq (19))
+
+    def step(self, hard, soft):
+        p, sc, nhp = self.p, self.sc, self.nhp
+        if self.reach:
+            p.render_obstacles(hard, None if not p.flags & 2 else soft)
+            p.reach_run(sc.start, self.n_cycles)
+            try:
+                self.plan = p.reach_extract_path(self.goal)
+            except nhp.NhpError as e:
+                if e.code != -5:
+                    raise
+                self.plan = ([], 0xFFFFFFFF)
+            return
+        if self.dt_dev:
+            p.render_obstacles_dt(hard, 4.0)                       # pipeline steps 1-4 on the device
+        else:
+            p.render_obstacles(hard, soft)
+        p.run_nturn(sc.start, self.n_cycles)
+        try:
+            self.plan = p.extract_path(self.goal)                  # synchronises; plan comes back to the host
+        except nhp.NhpError as e:
+            if e.code != -5:
+                raise
+            self.plan = ([], 0xFFFFFFFF)
+
+    def warm_up(self, n):
+        """Warm-up steps, then choose a goal the sweeps actually reach (fixed for all timed steps)."""
+        p, sc = self.p, self.sc
+        for _ in range(max(n, 1)):
+            self.step(self.hard_d, self.soft_d)
+        if self.reach:
+            K = p.reach_count_numpy()
+            cands = [tuple(sc.goal)] + [tuple(g) for g in sc.extra_goals]
+            reached = [g for g in cands if K[g[2], g[1], g[0]] != 255]
+            self.goal = reached[0] if K[sc.goal[2], sc.goal[1], sc.goal[0]] != 255 or not reached else max(reached, key=lambda g: K[g[2], g[1], g[0]])
+        else:
+            p.status()
+            self.goal = pick_goal(p, sc, self.torch)
+        self.step(self.hard_d, self.soft_d)
+
+    def timed(self, steps, host=False, profile=False):
+        """-> (device ms over `steps` steps, launches, {slot: (ms, launches)} if profile).  With `profile` every launch is
+        bracketed by an event pair and the pool is drained after EVERY step, so no launch goes untimed."""
+        p, torch = self.p, self.torch
+        hard, soft = (self.hard_h, self.soft_h) if host else (self.hard_d, self.soft_d)
+        p.kernel_times(reset=True)
+        p.set_profiling(profile)
+        l0 = p.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        self.replicas.barrier(); torch.cuda.synchronize()
+        e0.record()
+        for _ in range(steps):
+            self.step(hard, soft)
+            if profile:
+                p.kernel_times()
+        e1.record()
+        torch.cuda.synchronize(); self.replicas.barrier()
+        p.set_profiling(False)
+        kt = p.kernel_times(reset=True) if profile else None
+        return e0.elapsed_time(e1), p.launch_count() - l0, kt
+
+    def updates_per_launch(self, slot):
+        """Pose-updates one launch of `slot` processes (N_R per maneuver kernel)."""
+        nt = self.sc.nt
+        return {"turn_pair": 2 * self.n_r, "straight_xrows": self.n_r * self.nx // nt,
+                "straight_rows": self.n_r * (nt - self.nx) // nt}.get(slot, self.n_r)
+
+    def rooflines(self, kt, steps, step_ms, peak, config):
+        """Per sweep kernel: algorithmic bytes / CUDA-event time (`frac`, the 6-pass definition of SURVEY 8(d)) and the
+        committed ncu dram bytes / the same time (`frac_traffic`, the physical HBM fraction)."""
+        alg_b = ALG_BYTES_SOFT if self.sc.soft is not None else ALG_BYTES_HARD
+        out = {}
+        for k in SWEEP_SLOTS:
+            ms, n = kt.get(k, (0.0, 0))
+            if not n:
+                continue
+            avg = ms / n
+            alg = alg_b * self.updates_per_launch(k)
+            tr = measured_traffic(config, k)
+            ach = alg / (avg * 1e-3) / 1e9
+            out[k] = {"avg_launch_ms": avg, "launches_timed": int(n), "ms_per_step": ms / steps, "share_of_step": ms / steps / step_ms,
+                      "pose_updates_per_launch": self.updates_per_launch(k), "algorithmic_bytes_per_launch": alg,
+                      "achieved": ach, "frac": ach / peak,
+                      "traffic": tr["bytes_per_launch"] if tr else None, "traffic_source": tr["source"] if tr else None,
+                      "frac_traffic": (tr["bytes_per_launch"] / (avg * 1e-3) / 1e9 / peak) if tr else None}
+        return out
+
+    def close(self):
+        self.p.close()
+        del self.hard_d, self.soft_d, self.p
+        self.torch.cuda.empty_cache()
+
+
+def side_config(nhp, torch, replicas, dev, config, peak, flags=0, steps=2, cycles=0):
+    """One more workload (or the same one under NHP_FLAG_FIXED_WORK), timed the same way with fewer steps."""
+    import scenes
+    sc = scenes.CONFIGS[config](replicas.replica_seed(config, 0))
+    b = PlanBench(nhp, torch, replicas, sc, cycles or sc.n_cycles, dev, flags=flags)
+    b.warm_up(1)
+    ms, launches, _ = b.timed(steps)
+    ms_prof, _, kt = b.timed(steps, profile=True)
+    rl = b.rooflines(kt, steps, ms_prof / steps, peak, config)
+    dom = max(rl, key=lambda k: rl[k]["ms_per_step"]) if rl else None
+    out = {"workload": workload_name(sc, b.n_cycles), "baseline_config": config, "steps": steps, "ms_per_step": ms / steps,
+           "value": steps * b.updates_per_plan / (ms * 1e-3) / 1e9, "unit": UNIT, "plans_per_sec": steps / (ms * 1e-3),
+           "gpu_launches": int(launches), "plan_waypoints": len(b.plan[0]), "plan_cost": b.plan[1],
+           "dominant_kernel": dom,
+           "kernels": {k: {kk: v[kk] for kk in ("avg_launch_ms", "ms_per_step", "frac", "traffic", "frac_traffic")} for k, v in rl.items()},
+           "kernel_ms_per_step": {k: round(v[0] / steps, 4) for k, v in kt.items() if v[1] and k not in nhp.binding.NESTED_SLOTS}}
+    b.close()
+    return out
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) outside torchrun: launch the N ranks ourselves, one process per GPU."""
+    import socket
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.exit(subprocess.call(cmd))
+
+
 def run_ours(args):
+    if args.gpus > 1 and "RANK" not in os.environ:
+        respawn_under_torchrun(args)
     import torch
 
     import paper_2306_01301_b200 as nhp
@@ -143,108 +291,66 @@ def run_ours(args):
 
     rank, local_rank, ws = replicas.init("nccl")
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    assert ws == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE = {ws}"
+    assert local_rank < torch.cuda.device_count(), f"rank {rank}: only {torch.cuda.device_count()} GPU(s) visible"
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     sc = scenes.CONFIGS[args.config](replicas.replica_seed(args.config, rank))
     n_cycles = args.cycles or sc.n_cycles
-    n_r = sc.n * sc.n * sc.nt
-    updates_per_plan = 6 * n_cycles * n_r
-    p = nhp.Planner.from_scene(sc, flags=nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0, device=dev)
-    hard_d = torch.from_numpy(sc.hard).to(dev)
-    soft_d = torch.from_numpy(sc.soft).to(dev) if sc.soft is not None else None
-    hard_h = torch.from_numpy(sc.hard).pin_memory()
-    soft_h = torch.from_numpy(sc.soft).pin_memory() if sc.soft is not None else None
-    state = {"goal": tuple(sc.goal), "plan": None}
-
-    dt_dev = args.dt_on_device and sc.soft is not None
-
-    def step(hard, soft):
-        if args.reach:
-            p.render_obstacles(hard, None if not p.flags & 2 else soft)
-            p.reach_run(sc.start, n_cycles)
-            try:
-                state["plan"] = p.reach_extract_path(state["goal"])
-            except nhp.NhpError as e:
-                if e.code != -5:
-                    raise
-                state["plan"] = ([], 0xFFFFFFFF)
-            return
-        if dt_dev:
-            p.render_obstacles_dt(hard, 4.0)                       # pipeline steps 1-4 on the device
-        else:
-            p.render_obstacles(hard, soft)
-        p.run_nturn(sc.start, n_cycles)
-        try:
-            state["plan"] = p.extract_path(state["goal"])          # synchronises; plan comes back to the host
-        except nhp.NhpError as e:
-            if e.code != -5:
-                raise
-            state["plan"] = ([], 0xFFFFFFFF)
-
-    # warm-up, then choose a goal the sweeps actually reach (fixed for all timed steps)
-    for _ in range(max(args.warmup, 1)):
-        step(hard_d, soft_d)
-    if args.reach:
-        K = p.reach_count_numpy()
-        cands = [tuple(sc.goal)] + [tuple(g) for g in sc.extra_goals]
-        reached = [g for g in cands if K[g[2], g[1], g[0]] != 255]
-        state["goal"] = reached[0] if K[sc.goal[2], sc.goal[1], sc.goal[0]] != 255 or not reached else max(reached, key=lambda g: K[g[2], g[1], g[0]])
-        del K
-    else:
-        p.status()
-        state["goal"] = pick_goal(p, sc, torch)
-    step(hard_d, soft_d)
-
-    def timed(hard, soft, profile):
-        p.kernel_times(reset=True)
-        p.set_profiling(profile)
-        l0 = p.launch_count()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        replicas.barrier(); torch.cuda.synchronize()
-        e0.record()
-        for _ in range(args.steps):
-            step(hard, soft)
-        e1.record()
-        torch.cuda.synchronize(); replicas.barrier()
-        p.set_profiling(False)
-        return e0.elapsed_time(e1), p.launch_count() - l0
+    flags = (nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0) | (nhp.FLAG_FIXED_WORK if args.fixed_work else 0)
+    b = PlanBench(nhp, torch, replicas, sc, n_cycles, dev, flags=flags, reach=args.reach, dt_on_device=args.dt_on_device)
+    p, n_r, updates_per_plan, dt_dev = b.p, b.n_r, b.updates_per_plan, b.dt_dev
+    b.warm_up(args.warmup)
 
     clocks = ClockSampler(local_rank)
     if rank == 0:
         clocks.start()
-    ms_dev, launches = timed(hard_d, soft_d, False)
+    ms_dev, launches, _ = b.timed(args.steps)
     # the same K steps once more with an event pair around every launch: per-kernel durations for the roofline lines
     # (the events cost ~3 % of the step, so `value` is taken from the pass without them)
-    ms_prof, _ = timed(hard_d, soft_d, True)
-    kt = p.kernel_times(reset=True)
+    ms_prof, _, kt = b.timed(args.steps, profile=True)
+    dropped = p.prof_dropped()
     clk = clocks.stop() if rank == 0 else None
-    ms_e2e, _ = timed(hard_h, soft_h, False)
-    plan, cost = state["plan"]
+    ms_e2e, _, _ = b.timed(args.steps, host=True)
+    plan, cost = b.plan
     ms_dev_max, units = replicas.aggregate(ms_dev, args.steps * updates_per_plan, dev)
     ms_e2e_max, _ = replicas.aggregate(ms_e2e, 0, dev)
     if rank != 0:
-        p.close(); replicas.shutdown()
+        b.close(); replicas.shutdown()
         return
 
     peak, peak_src = peak_hbm()
-    alg_b = ALG_BYTES_SOFT if sc.soft is not None else ALG_BYTES_HARD
-    # sweep kernels by slot: a single maneuver per launch (N_R pose-updates), or a turn pair (RB+RF / LB+LF: 2 N_R)
-    sweeps = {k: v for k, v in kt.items() if (k in nhp.MANEUVER_NAMES or k == "turn_pair") and v[1]}
+    state = {"goal": b.goal, "plan": b.plan}
+    hard_h, soft_h = b.hard_h, b.soft_h
     if args.reach:
         return finish_reach(args, sc, n_cycles, n_r, ws, ms_dev_max, ms_e2e_max, units, launches, kt, clk, state, peak, peak_src, hard_h, p, replicas)
+    step_prof_ms = ms_prof / args.steps
+    if not any(kt.get(k, (0, 0))[1] for k in SWEEP_SLOTS):               # bring-up kernels: the maneuver slots themselves
+        rl = {}
+        sweeps = {k: v for k, v in kt.items() if k in nhp.MANEUVER_NAMES and v[1]}
+    else:
+        rl = b.rooflines(kt, args.steps, step_prof_ms, peak, args.config)
+        sweeps = {k: kt[k] for k in rl}
+    alg_b = ALG_BYTES_SOFT if sc.soft is not None else ALG_BYTES_HARD
     dom = max(sweeps, key=lambda k: sweeps[k][0])
     dom_ms, dom_n = sweeps[dom]
-    per_launch_bytes = alg_b * n_r * (2 if dom == "turn_pair" else 1)
+    dom_upd = b.updates_per_launch(dom)
+    per_launch_bytes = alg_b * dom_upd
     achieved = per_launch_bytes / (dom_ms / max(dom_n, 1) * 1e-3) / 1e9 if dom_ms > 0 else 0.0
     sweep_ms = sum(v[0] for v in sweeps.values())
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
-    traffic = measured_traffic(args.config, dom)
-    # secondary bound: the integer min/max pipe, 16 lanes per SM sub-partition and clock
-    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    dom_rl = rl.get(dom, {})
+    # physical HBM fraction of all sweeps together: committed ncu dram bytes per launch x launches / their summed time
+    tr_known = [k for k in rl if rl[k]["traffic"] is not None]
+    tr_bytes = sum(rl[k]["traffic"] * rl[k]["launches_timed"] for k in tr_known)
+    tr_ms = sum(sweeps[k][0] for k in tr_known)
+    # secondary bound: the integer min/max pipe, measured live by the library's micro-benchmark
     sm_clock = (clk or {}).get("sm_mhz") or 1965.0
-    alu_peak = sm_count * 4 * 16 * sm_clock * 1e6 / 1e12                       # T lane-ops / s
-    ops_per_update = 3 if dom in ("SF", "SB") else 5
-    alu_achieved = ops_per_update * n_r * (2 if dom == "turn_pair" else 1) / (dom_ms / max(dom_n, 1) * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    alu_ops, sm_count = p.microbench_alu(8)
+    alu_peak = alu_ops / 1e12                                                   # T lane-ops / s
+    ops_per_update = 3 if dom.startswith("straight") or dom in ("SF", "SB") else 5
+    alu_achieved = ops_per_update * dom_upd / (dom_ms / max(dom_n, 1) * 1e-3) / 1e12 if dom_ms > 0 else 0.0
+    top_level = {k: v for k, v in kt.items() if v[1] and k not in nhp.binding.NESTED_SLOTS}
     out = {
         "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
@@ -252,28 +358,44 @@ def run_ours(args):
         "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config,
                    "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)", "soft_image": ("device distance transform" if dt_dev else "harness (CPU)") if sc.soft is not None else None,
                    "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
-                   "goal": list(state["goal"]), "plan_waypoints": len(plan), "plan_cost": cost},
+                   "fixed_work": bool(args.fixed_work),
+                   "goal": list(b.goal), "plan_waypoints": len(plan), "plan_cost": cost},
         "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
         "clocks": clk,
         "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
                 "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if (soft_h is not None and not dt_dev) else 0)),
-                "d2h_bytes_per_step": int(16 * 4096 + 32)},
+                "d2h_bytes_per_step": int(4 * 16 + 16 * max(len(plan), 128))},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": n_r * (2 if dom == "turn_pair" else 1), "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic["bytes_per_launch"] if traffic else None,
-                     "traffic_source": traffic["source"] if traffic else None, "peak_source": peak_src,
+        "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": dom_upd, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                     "frac": achieved / peak, "traffic": dom_rl.get("traffic"), "frac_traffic": dom_rl.get("frac_traffic"),
+                     "traffic_source": dom_rl.get("traffic_source"), "peak_source": peak_src,
+                     "frac_definition": "frac = SURVEY 8(d) algorithmic bytes (8.125 B, 9.125 B soft, per pose-update; a fused pair launch is charged "
+                                        "two maneuvers) / CUDA-event time / peak: above 1 because one read of V serves up to four laps; "
+                                        "frac_traffic = ncu dram bytes per launch (profiles/traffic.csv) / the same time / peak: the physical HBM fraction",
                      "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
-                     "launches_timed": int(dom_n),
-                     "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps}},
+                     "launches_timed": int(dom_n), "launches_untimed": int(dropped),
+                     "kernels": rl,
+                     "all_sweeps": {"achieved": sweep_gbs, "frac": sweep_gbs / peak, "ms_per_step": sweep_ms / args.steps,
+                                    "traffic_per_step": tr_bytes / args.steps if tr_known else None,
+                                    "frac_traffic": (tr_bytes / (tr_ms * 1e-3) / 1e9 / peak) if tr_known and tr_ms > 0 else None}},
         "alu": {"bound": "alu", "kernel": dom, "achieved": alu_achieved, "peak": alu_peak, "unit": "T min/max lane-ops/s",
                 "frac": alu_achieved / alu_peak, "ops_per_pose_update": ops_per_update,
-                "peak_source": f"{sm_count} SMs x 4 x 16 lanes x {sm_clock:.0f} MHz (DESIGN.md 6.7)"},
-        "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in kt.items() if v[1]},
-        "ms_per_step_with_kernel_events": ms_prof / args.steps,
+                "peak_source": f"nhp_microbench_alu, measured in this run: 8 independent VIADDMNMX chains per thread, 8 warps per sub-partition, "
+                               f"{sm_count} SMs = {alu_ops / (sm_count * 4 * sm_clock * 1e6):.2f} lane-ops per sub-partition and clock at {sm_clock:.0f} MHz (DESIGN.md 6.7)"},
+        "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in top_level.items()},
+        "kernel_ms_sum": sum(v[0] for v in top_level.values()) / args.steps,
+        "ms_per_step_with_kernel_events": step_prof_ms,
     }
+    b.close()
+    if ws == 1 and not args.no_extra:
+        # T12 ("run time independent of scene"): the same workload with the data-dependent short cuts off
+        if not args.fixed_work and not args.simple_kernels:
+            fw = side_config(nhp, torch, replicas, dev, args.config, peak, flags=nhp.FLAG_FIXED_WORK, steps=min(args.steps, 3), cycles=args.cycles)
+            out["fixed_work"] = {k: fw[k] for k in ("ms_per_step", "value", "unit", "plans_per_sec", "steps", "kernels")}
+        # the soft-cost path and the largest grid, one short timed run each (BASELINE.json configs 4 and 5)
+        out["other_configs"] = [side_config(nhp, torch, replicas, dev, c, peak, steps=2) for c in (4, 5) if c != args.config]
     if not args.no_cpu_baseline and ws == 1:
         out["cpu_baseline"] = cpu_baseline(sc, n_cycles, sample_cycles=2)
-    p.close()
     replicas.shutdown()
     print(json.dumps(out), flush=True)
 
@@ -319,7 +441,8 @@ def oracle_setup(sc):
 def cpu_baseline(sc, n_cycles, sample_cycles=2):
     """The oracle as it stands on this box's host cores, on a bounded sample of the same workload: its own
     rendering of the scene plus `sample_cycles` of the N_T maneuver cycles over the full volume.  The value is
-    plan-equivalent: sampled pose-updates / (sweep time + render time * sample_cycles / N_T)."""
+    plan-equivalent: sampled pose-updates / (sweep time + render time * sample_cycles / N_T).  `single_thread` is the
+    same oracle on ONE thread (the configuration of the paper's CPU rows) over two maneuver sweeps."""
     import numpy as np
     o, Cv, Sv, t_render = oracle_setup(sc)
     V = np.full(o.shape, 0xFFFFFFFF, np.uint32)
@@ -328,11 +451,20 @@ def cpu_baseline(sc, n_cycles, sample_cycles=2):
     o.cycles(V, Cv, Sv, sample_cycles)
     t_sweeps = time.perf_counter() - t0
     upd = 6 * sample_cycles * V.size
-    return {"value": upd / (t_sweeps + t_render * sample_cycles / n_cycles) / 1e9, "unit": UNIT, "cores": int(o.threads),
+    cores = int(o.threads)
+    o.set_threads(1)
+    t0 = time.perf_counter()
+    o.sweep(0, V, Cv, Sv)                              # LF: a turn maneuver (two laps)
+    o.sweep(1, V, Cv, Sv)                              # SF: a straight maneuver
+    t_one = time.perf_counter() - t0
+    return {"value": upd / (t_sweeps + t_render * sample_cycles / n_cycles) / 1e9, "unit": UNIT, "cores": cores,
             "kind": "oracle",
             "sample": f"oracle render of the full scene ({t_render:.2f} s) + {sample_cycles} of {n_cycles} maneuver cycles "
                       f"over the full {sc.n}x{sc.n}x{sc.nt} volume ({t_sweeps:.2f} s), OpenMP over curves on all host cores; "
-                      f"render time charged pro rata"}
+                      f"render time charged pro rata",
+            "single_thread": {"value": 2 * V.size / t_one / 1e9, "unit": UNIT, "cores": 1,
+                              "sample": f"one turn sweep (LF) + one straight sweep (SF) over the full volume on one thread ({t_one:.2f} s), "
+                                        f"sweeps only (no render)"}}
 
 
 def run_reference(args):

@@ -288,12 +288,21 @@ long long nhp_launch_count(const nhp_planner *p);
  *   slot 9      back-tracking (a7), slot 10 footprint rasterisation + image packing,
  *   slot 11     turn-pair launches (RB+RF or LB+next LF in one kernel: two maneuvers per launch)
  *   slot 12     distance transform + soft-image synthesis (nhp_render_obstacles_dt)
- *   slot 13     one level of the reachability planner (all its launches: copy, six sweeps, transpositions) */
-#define NHP_KERNEL_SLOTS 14
+ *   slot 13     one level of the reachability planner (all its launches: copy, six sweeps, transpositions)
+ *   slot 14     the I = 0 ("x-rows") kernel of a straight maneuver alone, slot 15 its I = 1 ("rows") kernel alone: both are
+ *               NESTED inside the SF / SB pair of slots 1 and 4 (do not add them to a sum over the slots) */
+#define NHP_KERNEL_SLOTS 16
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
 /* Launches that ran untimed since creation because the event pool was exhausted (0 in any sane use). */
 long long nhp_prof_dropped(const nhp_planner *p);
+
+/* Integer-pipe micro-benchmark behind bench.py's `alu` line: launches a kernel of `chains`
+ * (1..8) independent VIADDMNMX (add + min, the instruction every sweep step is made of) dependency chains per thread on the
+ * handle's stream, 8 warps per SM sub-partition on every SM, times it with CUDA events and returns the throughput in
+ * lane-operations per second (*lane_ops_per_s) and the SM count used (*sms).  Touches none of the planner's volumes.
+ * Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_CUDA. */
+int nhp_microbench_alu(nhp_planner *p, int chains, double *lane_ops_per_s, int *sms);
 
 #ifdef __cplusplus
 }

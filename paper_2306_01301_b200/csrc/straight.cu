@@ -348,11 +348,11 @@ int launch_straight_tile(nhp_planner *p, int m)
     const int fwd = (m == M_SF);
     const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : 0;
     if (soft) {
-        straight_xrows_kernel<true><<<gx, xwarps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
-        straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        { ProfScope px(p, 14); straight_xrows_kernel<true><<<gx, xwarps * 32, smem, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed); }
+        { ProfScope py(p, 15); straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed); }
     } else {
-        straight_xrows_kernel<false><<<gx, xwarps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
-        straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        { ProfScope px(p, 14); straight_xrows_kernel<false><<<gx, xwarps * 32, smem, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed); }
+        { ProfScope py(p, 15); straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed); }
     }
     return 2;
 }
