@@ -46,6 +46,7 @@ def parse_args():
     ap.add_argument("--reach", action="store_true",
                     help="time the reachability (bit-vector) planner of appendix C instead: render + N_T levels + back-track")
     ap.add_argument("--fixed-work", action="store_true", help="NHP_FLAG_FIXED_WORK: data-dependent short cuts off (PAPER.md:565)")
+    ap.add_argument("--no-shortcuts", action="store_true", help="NHP_FLAG_NO_SHORTCUTS: every warp runs every pass; stores still only where a value improved")
     ap.add_argument("--no-extra", action="store_true", help="skip the fixed-work pass and the configs 4 / 5 side runs")
     ap.add_argument("--dt-on-device", action="store_true",
                     help="soft configs: distance transform + soft image on the GPU (nhp_render_obstacles_dt) instead of the harness image")
@@ -65,7 +66,7 @@ def measured_traffic(config, slot):
                 if ln.startswith("#") or not ln.strip():
                     continue
                 c, k, b, src = ln.strip().split(",")
-                if int(c) == config and k == slot:
+                if c == str(config) and k == slot:
                     return {"bytes_per_launch": int(b), "source": src}
     except OSError:
         pass
@@ -249,7 +250,7 @@ class PlanBench:
         self.torch.cuda.empty_cache()
 
 
-def side_config(nhp, torch, replicas, dev, config, peak, flags=0, steps=2, cycles=0):
+def side_config(nhp, torch, replicas, dev, config, peak, flags=0, steps=2, cycles=0, traffic_key=None):
     """One more workload (or the same one under NHP_FLAG_FIXED_WORK), timed the same way with fewer steps."""
     import scenes
     sc = scenes.CONFIGS[config](replicas.replica_seed(config, 0))
@@ -257,7 +258,7 @@ def side_config(nhp, torch, replicas, dev, config, peak, flags=0, steps=2, cycle
     b.warm_up(1)
     ms, launches, _ = b.timed(steps)
     ms_prof, _, kt = b.timed(steps, profile=True)
-    rl = b.rooflines(kt, steps, ms_prof / steps, peak, config)
+    rl = b.rooflines(kt, steps, ms_prof / steps, peak, traffic_key or config)
     dom = max(rl, key=lambda k: rl[k]["ms_per_step"]) if rl else None
     out = {"workload": workload_name(sc, b.n_cycles), "baseline_config": config, "steps": steps, "ms_per_step": ms / steps,
            "value": steps * b.updates_per_plan / (ms * 1e-3) / 1e9, "unit": UNIT, "plans_per_sec": steps / (ms * 1e-3),
@@ -297,7 +298,7 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank)
     sc = scenes.CONFIGS[args.config](replicas.replica_seed(args.config, rank))
     n_cycles = args.cycles or sc.n_cycles
-    flags = (nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0) | (nhp.FLAG_FIXED_WORK if args.fixed_work else 0)
+    flags = (nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0) | (nhp.FLAG_FIXED_WORK if args.fixed_work else 0) | (nhp.FLAG_NO_SHORTCUTS if args.no_shortcuts else 0)
     b = PlanBench(nhp, torch, replicas, sc, n_cycles, dev, flags=flags, reach=args.reach, dt_on_device=args.dt_on_device)
     p, n_r, updates_per_plan, dt_dev = b.p, b.n_r, b.updates_per_plan, b.dt_dev
     b.warm_up(args.warmup)
@@ -358,7 +359,7 @@ def run_ours(args):
         "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config,
                    "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)", "soft_image": ("device distance transform" if dt_dev else "harness (CPU)") if sc.soft is not None else None,
                    "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
-                   "fixed_work": bool(args.fixed_work),
+                   "fixed_work": bool(args.fixed_work), "no_shortcuts": bool(args.no_shortcuts),
                    "goal": list(b.goal), "plan_waypoints": len(plan), "plan_cost": cost},
         "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
         "clocks": clk,
@@ -389,9 +390,12 @@ def run_ours(args):
     b.close()
     if ws == 1 and not args.no_extra:
         # T12 ("run time independent of scene"): the same workload with the data-dependent short cuts off
-        if not args.fixed_work and not args.simple_kernels:
-            fw = side_config(nhp, torch, replicas, dev, args.config, peak, flags=nhp.FLAG_FIXED_WORK, steps=min(args.steps, 3), cycles=args.cycles)
-            out["fixed_work"] = {k: fw[k] for k in ("ms_per_step", "value", "unit", "plans_per_sec", "steps", "kernels")}
+        if not args.fixed_work and not args.no_shortcuts and not args.simple_kernels:
+            for key, fl, cfgkey in (("no_shortcuts", nhp.FLAG_NO_SHORTCUTS, f"{args.config}:no_shortcuts"), ("fixed_work", nhp.FLAG_FIXED_WORK, f"{args.config}:fixed_work")):
+                fw = side_config(nhp, torch, replicas, dev, args.config, peak, flags=fl, steps=min(args.steps, 3), cycles=args.cycles, traffic_key=cfgkey)
+                out[key] = {k: fw[k] for k in ("ms_per_step", "value", "unit", "plans_per_sec", "steps", "kernels")}
+            out["no_shortcuts"]["what"] = "NHP_FLAG_NO_SHORTCUTS: every warp runs every pass of every sweep; vertices written only where they improved"
+            out["fixed_work"]["what"] = "NHP_FLAG_FIXED_WORK: no short cuts and every visited vertex written back (the paper's unconditional store): same instructions and bytes whatever the scene holds"
         # the soft-cost path and the largest grid, one short timed run each (BASELINE.json configs 4 and 5)
         out["other_configs"] = [side_config(nhp, torch, replicas, dev, c, peak, steps=2) for c in (4, 5) if c != args.config]
     if not args.no_cpu_baseline and ws == 1:

@@ -51,7 +51,11 @@ extern "C" {
 #define NHP_FLAG_FIXED_WORK 8     /* switch off the data-dependent short cuts of the sweeps (warps whose vertices are all
                                      blocked / hold no finite value yet skip their chains): every launch then executes
                                      the same instructions whatever the scene holds ("run time independent of scene",
-                                     PAPER.md:39, l.565).  Same results; for measuring the fixed-work time */
+                                     PAPER.md:39, l.565) AND stores every vertex it visits, as the paper's loop does
+                                     (V[i] = min(v, u) unconditionally, Insert 5 l.948): same instructions and same bytes.
+                                     Same results; for measuring the fixed-work time */
+#define NHP_FLAG_NO_SHORTCUTS 16  /* only the first half of NHP_FLAG_FIXED_WORK: every warp runs every pass of every sweep, but a
+                                     vertex is still written back only where its value improved.  Same results */
 
 #define NHP_DEFAULT_CYCLES 8      /* PAPER.md:392 "our default is 8 cycles" (n_cycles <= 0 selects it) */
 

@@ -116,6 +116,33 @@ int upload_tables(nhp_planner *p)
     CU(cudaMemcpyAsync(p->d_lenq, p->len_q.data(), sizeof(uint32_t) * 6 * nt, cudaMemcpyHostToDevice, p->stream));
     CU(cudaMemcpyAsync(p->d_IJ, IJ.data(), nt, cudaMemcpyHostToDevice, p->stream));
     CU(cudaMemcpyAsync(p->d_rot, rot.data(), sizeof(int32_t) * 4 * nt, cudaMemcpyHostToDevice, p->stream));
+    // x-rows kernel (straight.cu: straight_xl_kernel): what tile T (columns 32 T .. 32 T + 31) of an I = 0 slice needs that depends
+    // only on (slice, T).  delta_k = B(32 T + k) - bmin is the row of line 0 at column k relative to the tile's first row; the
+    // 8-column sector group m = k / 8 is fetched sheared by dlo8(m) = its smallest delta.  Word of lane k:
+    //     dq_k = delta_k - dlo8(m)  (bits 0-2)  |  rows the group needs = 32 + max dq  (bits 8-13)  |  bmin + dlo8(m)  (bits 16-31, signed)
+    std::vector<uint32_t> xl;
+    if (n >= 32) {
+        const int NT = n / 32, nx = p->n_xslices;
+        xl.assign((size_t)nx * NT * 32, 0u);
+        for (int xs = 0; xs < nx; xs++) {
+            const int32_t *Bt = p->B.data() + (size_t)tlist[xs] * n;
+            for (int T = 0; T < NT; T++) {
+                int bmin = 1 << 30;
+                for (int k = 0; k < 32; k++) bmin = Bt[32 * T + k] < bmin ? Bt[32 * T + k] : bmin;
+                for (int m8 = 0; m8 < 4; m8++) {
+                    int lo = 1 << 30, hi = -(1 << 30);
+                    for (int e = 0; e < 8; e++) { const int d = Bt[32 * T + 8 * m8 + e] - bmin; lo = d < lo ? d : lo; hi = d > hi ? d : hi; }
+                    if (hi - lo > 7 || bmin + lo < -32768 || bmin + lo > 32767) return fail(p, NHP_E_ARG, "x-rows table: slope of a straight line exceeds 1");
+                    for (int e = 0; e < 8; e++) {
+                        const int k = 8 * m8 + e, dq = Bt[32 * T + k] - bmin - lo;
+                        xl[((size_t)xs * NT + T) * 32 + k] = (uint32_t)dq | ((uint32_t)(32 + hi - lo) << 8) | ((uint32_t)(bmin + lo) << 16);
+                    }
+                }
+            }
+        }
+        CU(cudaMalloc(&p->d_xl_tab, sizeof(uint32_t) * xl.size() + 16));
+        CU(cudaMemcpyAsync(p->d_xl_tab, xl.data(), sizeof(uint32_t) * xl.size(), cudaMemcpyHostToDevice, p->stream));
+    }
     CU(cudaStreamSynchronize(p->stream));            // the staging vectors die with this scope
     return NHP_OK;
 }
@@ -282,7 +309,7 @@ int nhp_planner_destroy(nhp_planner *p)
     {
         DeviceGuard guard(p);
         cudaStreamSynchronize(p->stream);
-        cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist);
+        cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist); cudaFree(p->d_xl_tab);
         cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_status); cudaFree(p->d_dtg); cudaFree(p->d_goals);
         if (p->h_status) cudaFreeHost(p->h_status);
         for (auto &e : p->ev) if (e) cudaEventDestroy(e);

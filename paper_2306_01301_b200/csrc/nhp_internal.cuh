@@ -93,6 +93,7 @@ struct nhp_planner {
     uint8_t *d_IJ = nullptr;
     int16_t *d_tlist = nullptr;    // [nt] slices with I = 0 first (n_xslices of them), then those with I = 1
     int n_xslices = 0;
+    uint32_t *d_xl_tab = nullptr;  // [n_xslices][n/32][32] tile word of every lane of the x-rows kernel (straight.cu: straight_xl_kernel)
     int32_t *d_rot = nullptr;      // [nt][4] cosq, sinq, 2*Psi0, 2*Psi1
     // footprint (all in the caller's workspace, sized for lim.max_footprint_radius)
     int rad = 0, side = 0, sidew = 0;

@@ -459,7 +459,7 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
             for (int k = 0; k < L; k++) checksum_add(after, col[k], one);
         }
     }
-    if (after != before || fixed) {
+    if (after != before || fixed == 1) {
         int row0 = sec * L;
         asm volatile("" : "+r"(row0));        // re-read the row table: keeping the addresses alive across the passes spills
         if (!wraps) tile_rows_store<L, false>(col, V, so + row0, lane, (uint32_t)mx);
@@ -491,7 +491,7 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     };
     const TurnPass pa = pass(ma), pb = pass(mb);
     const uint8_t *Sc = left ? p->S_left : p->S_right;
-    const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : 0;
+    const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : (p->w.flags & NHP_FLAG_NO_SHORTCUTS) ? 2 : 0;   // 1: no short cuts, store all; 2: no short cuts
     const dim3 grid(n / 32, n), block(32 * S);
     const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 4 * (size_t)S * 32;
     ProfScope prof(p, mb >= 0 ? 11 : ma);

@@ -40,7 +40,7 @@ def small_scenes():
     ]
 
 
-@pytest.mark.parametrize("flags", [0, 4, 8])     # tile kernels, thread-per-curve kernels, NHP_FLAG_FIXED_WORK (short cuts off)
+@pytest.mark.parametrize("flags", [0, 4, 8, 16])     # tile kernels, thread-per-curve kernels, NHP_FLAG_FIXED_WORK, NHP_FLAG_NO_SHORTCUTS
 def test_tables_render_sweeps_and_plans_match_the_oracle(mods, flags):
     oracle, nhp = mods
     for sc in small_scenes():
