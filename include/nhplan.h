@@ -54,6 +54,11 @@ extern "C" {
                                      PAPER.md:39, l.565) AND stores every vertex it visits, as the paper's loop does
                                      (V[i] = min(v, u) unconditionally, Insert 5 l.948): same instructions and same bytes.
                                      Same results; for measuring the fixed-work time */
+#define NHP_FLAG_SECTIONS 32      /* straight sweeps by Sections (appendix D: one warp per 32-step section of a line, all
+                                     sections of a line at once, summary / ripple / apply) also on grids of more than 256 cells per side,
+                                     where the streaming kernels are the default (at most 512 cells: 16 sections).  Same results */
+#define NHP_FLAG_NO_SECTIONS 64   /* straight sweeps by the streaming kernels (one warp walks a whole band of lines) also on grids of at most
+                                     256 cells per side, where Sections are the default.  Same results */
 #define NHP_FLAG_NO_SHORTCUTS 16  /* only the first half of NHP_FLAG_FIXED_WORK: every warp runs every pass of every sweep, but a
                                      vertex is still written back only where its value improved.  Same results */
 

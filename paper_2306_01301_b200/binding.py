@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libnhplan.so")
 
 INF = 0xFFFFFFFF
-FLAG_FORWARD_ONLY, FLAG_SOFT, FLAG_SIMPLE_KERNELS, FLAG_FIXED_WORK, FLAG_NO_SHORTCUTS = 1, 2, 4, 8, 16
+FLAG_FORWARD_ONLY, FLAG_SOFT, FLAG_SIMPLE_KERNELS, FLAG_FIXED_WORK, FLAG_NO_SHORTCUTS, FLAG_SECTIONS, FLAG_NO_SECTIONS = 1, 2, 4, 8, 16, 32, 64
 DEFAULT_CYCLES = 8                                          # NHP_DEFAULT_CYCLES
 PLAN_EAGER = 128                                            # waypoints that come back with the status words (NHP_PLAN_EAGER)
 MANEUVER_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB")

@@ -298,6 +298,7 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
         if (cudaMemsetAsync(p->d_status, 0, 2 * sp_bytes, p->stream) != cudaSuccess) rc = NHP_E_CUDA;
     }
     if (rc == NHP_OK) rc = set_kernel_attributes(p);
+    if (rc == NHP_OK) rc = build_cycle_graph(p);
     if (rc != NHP_OK) { nhp_planner_destroy(p); return rc; }
     *out = p;
     return NHP_OK;
@@ -309,6 +310,8 @@ int nhp_planner_destroy(nhp_planner *p)
     {
         DeviceGuard guard(p);
         cudaStreamSynchronize(p->stream);
+        if (p->cycle_exec) cudaGraphExecDestroy(p->cycle_exec);
+        if (p->cycle_graph) cudaGraphDestroy(p->cycle_graph);
         cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist); cudaFree(p->d_xl_tab);
         cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_status); cudaFree(p->d_dtg); cudaFree(p->d_goals);
         if (p->h_status) cudaFreeHost(p->h_status);

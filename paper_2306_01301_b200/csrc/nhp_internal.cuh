@@ -128,6 +128,11 @@ struct nhp_planner {
     int plan_cap = 0, plan_eager = 128;    // waypoints brought back together with the status words (NHP_PLAN_EAGER)
     int32_t *h_status = nullptr;   // pinned: NHP_STATUS_WORDS words, then plan_cap waypoints
     nhp_waypoint *h_plan = nullptr;
+    // CUDA graph of one inner maneuver cycle (sweep.cu: build_cycle_graph), instantiated at creation for grids small enough
+    // for the launch overhead to matter; replayed by launch_cycles unless per-kernel profiling is on
+    cudaGraph_t cycle_graph = nullptr;
+    cudaGraphExec_t cycle_exec = nullptr;
+    int cycle_graph_kernels = 0;
     std::string err = "ok";
     long long launches = 0;
     // per-kernel timing (nhp_set_profiling): event pairs on the launching stream, drained at sync points
@@ -186,6 +191,7 @@ int launch_render(nhp_planner *p, bool soft);
 int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);
 int launch_cycles(nhp_planner *p, int n_cycles);
+int build_cycle_graph(nhp_planner *p);               // at creation; NHP_OK also when no graph is built
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);     // gi < 0: the goal comes from launch_goal_search
 int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w);
 int launch_seed_in_progress(nhp_planner *p, int m0);

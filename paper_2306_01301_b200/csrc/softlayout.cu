@@ -3,9 +3,11 @@
 // A sweep kernel walks along curves; its value volume V is staged tile by tile (sweep.cu, straight.cu), but the
 // soft multiplier S is one BYTE per vertex, too narrow to stage the same way (cp.async moves >= 4 bytes, and a warp
 // reading one byte per plane fetches a 32-byte sector for it).  So the renderer also writes S in the order the
-// sweeps consume it -- 32 consecutive steps of one curve are 32 consecutive bytes:
-//   S_left [y'][x'][Theta] = S[Theta][(y' + beta3(Theta)) & M][(x' + beta0(Theta)) & M]      left-turn curves, eq (18)
-//   S_right[y'][x'][Theta] = S[Theta][(y' + beta1(Theta)) & M][(x' + beta2(Theta)) & M]      right-turn curves, eq (18)
+// sweeps consume it:
+//   S_left [y'][x' / 32][Theta / 4][x' % 32][Theta % 4] = S[Theta][(y' + beta3(Theta)) & M][(x' + beta0(Theta)) & M]     left-turn curves, eq (18)
+//   S_right[y'][x' / 32][Theta / 4][x' % 32][Theta % 4] = S[Theta][(y' + beta1(Theta)) & M][(x' + beta2(Theta)) & M]     right-turn curves, eq (18)
+//       (tile-major: the four bytes of four consecutive planes of one curve are one word, the 32 curves of a turn tile lie next to
+//       each other, so a warp of the tile kernel reads one 128-byte line per four planes)
 //   S_line [Theta][x'][y'] = S at the vertex eq (23) gives for (x', y', Theta)                straight lines
 // Same bytes, same traffic per pose-update (1 B), three more volumes of N_R bytes in the caller's workspace.
 #include "nhp_internal.cuh"
@@ -15,8 +17,8 @@
 __global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
                                                               const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
 {
-    extern __shared__ __align__(16) uint8_t tile[];             // [32][nt + 16]
-    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2, stride = nt + 16;
+    extern __shared__ __align__(16) uint8_t tile[];             // [32][nt + 4]: an odd number of words per curve
+    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2, stride = nt + 4;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
     for (int t = warp; t < nt; t += nwarps) {
@@ -24,11 +26,11 @@ __global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restri
         tile[lane * stride + t] = S[((((size_t)t << log2_n) + ((yp + bb) & mx)) << log2_n) + ((x0 + ba + lane) & mx)];
     }
     __syncthreads();
-    const int chunks = nt >> 4;                                 // 16-byte chunks per curve
-    uint8_t *out = Sout + (((size_t)yp << log2_n) + x0) * nt;
-    for (int c = threadIdx.x; c < 32 * chunks; c += blockDim.x) {
-        const int curve = c / chunks, q = c - curve * chunks;
-        *(uint4 *)(out + (size_t)curve * nt + 16 * q) = *(const uint4 *)(tile + curve * stride + 16 * q);
+    // tile-major: word j = planes 4 j .. 4 j + 3 of a curve, the 32 curves of the tile next to each other (one 128-byte line)
+    uint32_t *out = (uint32_t *)Sout + (((size_t)yp << (log2_n - 5)) + blockIdx.x) * ((size_t)nt * 8);
+    for (int c = threadIdx.x; c < 8 * nt; c += blockDim.x) {
+        const int j = c >> 5, curve = c & 31;
+        out[c] = *(const uint32_t *)(tile + curve * stride + 4 * j);
     }
 }
 
@@ -64,7 +66,7 @@ __global__ void __launch_bounds__(256) soft_line_layout_kernel(uint8_t *__restri
 int launch_soft_layouts(nhp_planner *p)
 {
     const int n = p->n, nt = p->nt;
-    const size_t smem = (size_t)32 * (nt + 16);
+    const size_t smem = (size_t)32 * (nt + 4);
     soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
     soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
     soft_line_layout_kernel<<<dim3(n / 32, n / 32, nt), dim3(32, 8), 0, p->stream>>>(p->S_line, p->S, p->d_B, p->d_IJ, p->log2_n);

@@ -45,6 +45,7 @@ struct RelaxLoop {
         if (out != u) cm |= 1u << k;                                  // out <= u always
         line[k] = out;
         t = nhp_gate(t, u);
+        if (!SOFT) wp = w;                                            // (only the first step can be entered with another pending weight)
         if (SOFT) {
             const uint4 &q = (k < 16) ? s0 : s1;
             const uint32_t word = ((k >> 2) & 3) == 0 ? q.x : ((k >> 2) & 3) == 1 ? q.y : ((k >> 2) & 3) == 2 ? q.z : q.w;
@@ -160,6 +161,31 @@ constexpr int XL_STAGE = XL_DATA + 32 + 1;                 // + the 32 stage byt
 #ifndef XL_MINB_V
 #define XL_MINB_V 20
 #endif
+
+// gather / scatter the 32 columns of this thread's line from / to the staged tile: `row` points at the thread's stage row, offs4 at
+// the table of the columns' byte offsets (dq_k rows down, k words across; warp-uniform, read four at a time)
+__device__ __forceinline__ void xr_gather0(uint32_t (&u)[32], const char *row, const uint4 *offs4)
+{
+#pragma unroll
+    for (int q = 0; q < 8; q++) {
+        const uint4 o = offs4[q];
+        u[4 * q + 0] = *(const uint32_t *)(row + o.x);
+        u[4 * q + 1] = *(const uint32_t *)(row + o.y);
+        u[4 * q + 2] = *(const uint32_t *)(row + o.z);
+        u[4 * q + 3] = *(const uint32_t *)(row + o.w);
+    }
+}
+__device__ __forceinline__ void xr_scatter0(const uint32_t (&u)[32], char *row, const uint4 *offs4, uint32_t cm)
+{
+#pragma unroll
+    for (int q = 0; q < 8; q++) {
+        const uint4 o = offs4[q];
+        if ((cm >> (4 * q + 0)) & 1u) *(uint32_t *)(row + o.x) = u[4 * q + 0];
+        if ((cm >> (4 * q + 1)) & 1u) *(uint32_t *)(row + o.y) = u[4 * q + 1];
+        if ((cm >> (4 * q + 2)) & 1u) *(uint32_t *)(row + o.z) = u[4 * q + 2];
+        if ((cm >> (4 * q + 3)) & 1u) *(uint32_t *)(row + o.w) = u[4 * q + 3];
+    }
+}
 
 // tile word of a lane (api.cu: upload_tables): dq | rows << 8 | (bmin + dlo8) << 16.  LOG2N > 0: the grid size is a compile-time
 // constant, so the rows are immediate offsets from one base address as long as no lane's rows run across the seam j = N-1 -> 0
@@ -355,6 +381,133 @@ __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restr
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Sections for the straight sweeps (appendix D, Inserts 3-5): one CTA = one band of 32 neighbouring
+// lines, one WARP = one section = one tile of 32 sweep steps, all tiles of the band resident at once.
+//   pass 1  every warp sweeps its tile from v = infinity: (M, D) = the value arriving behind the tile and the summed edge cost
+//           across it (>= D_CAP if a blocked vertex interrupts it) -- (Sv, Sd) of Insert 3, l.923-928
+//   ripple  carry into section s = fold of the sections before it in travel order, (c, D, M) -> min(c + D, M), Insert 4
+//           l.935-939; the first section starts from infinity (the wall cell, DESIGN R12)
+//   pass 2  every warp sweeps its tile again from its carry (Insert 5, l.946-949)
+// (min, saturating +) is associative (DESIGN R18): bit-identical to the walk of the streaming kernels above.  A line of N
+// cells is N / 32 independent loads instead of N / 32 loads one after the other, which is what a small grid needs
+// ("not as much parallelism exposed as we could take advantage of"): at N = 256 a launch of the
+// streaming kernels is 1024 warps that each wait for 8 tiles in turn.  Used for N <= 256 (and on request: NHP_FLAG_SECTIONS);
+// from 512 cells on the streaming kernels already fill the machine and read each tile once without a barrier.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t SX_D_CAP = 1u << 31;
+
+template <bool UP, bool SOFT, int S = 0>
+struct SummaryLoop {
+    static __device__ __forceinline__ void run(const uint32_t *line, uint32_t &t, uint32_t &wp, uint32_t &d, uint32_t w, const uint4 &s0, const uint4 &s1)
+    {
+        constexpr int k = UP ? S : 31 - S;
+        const uint32_t u = line[k];
+        t = nhp_gate(nhp_arrive(t, wp, u), u);
+        if (!SOFT) wp = w;
+        if (SOFT) {
+            const uint4 &q = (k < 16) ? s0 : s1;
+            const uint32_t word = ((k >> 2) & 3) == 0 ? q.x : ((k >> 2) & 3) == 1 ? q.y : ((k >> 2) & 3) == 2 ? q.z : q.w;
+            wp = nhp_soft_weight(w, word, k & 3);
+            d += wp;
+        }
+        SummaryLoop<UP, SOFT, S + 1>::run(line, t, wp, d, w, s0, s1);
+    }
+};
+template <bool UP, bool SOFT>
+struct SummaryLoop<UP, SOFT, 32> {
+    static __device__ __forceinline__ void run(const uint32_t *, uint32_t &, uint32_t &, uint32_t &, uint32_t, const uint4 &, const uint4 &) {}
+};
+
+template <bool XS, bool SOFT>
+__global__ void __launch_bounds__(512) straight_sect_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline, const int16_t *__restrict__ B,
+                                                            const uint32_t *__restrict__ xl_tab, const uint8_t *__restrict__ IJ,
+                                                            const int16_t *__restrict__ tlist, const uint32_t *__restrict__ lenq, uint32_t ct,
+                                                            int log2_n, int is_forward, int fixed)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    const int n = 1 << log2_n, mx = n - 1, NT = n >> 5;
+    const int xs = blockIdx.y, t = tlist[xs];
+    const int lane = threadIdx.x & 31, T = threadIdx.x >> 5;                    // warp = tile T of the band
+    const int X0 = blockIdx.x << 5;
+    const bool up = (is_forward == ((IJ[t] >> 1) & 1));                         // eq (24)
+    unsigned long long Vt = (unsigned long long)(V + ((size_t)t << (2 * log2_n)));
+    asm volatile("" : "+l"(Vt));
+    uint2 *sMD = (uint2 *)smem;                                                 // [NT][32]
+    uint32_t *stage = smem + 2 * 32 * NT + T * XL_STAGE;                        // x-slices only
+    const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
+    uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
+    if (SOFT) {
+        const uint8_t *Sl = Sline + ((size_t)t << (2 * log2_n)) + ((size_t)(X0 + lane) << log2_n) + 32 * T;
+        s0 = ld_nc16(Sl); s1 = ld_nc16(Sl + 16);
+    }
+    uint32_t u[32];
+    uint32_t tw = 0;
+    int bmine = 0;
+    char *row = (char *)(stage + lane * XL_PITCH);
+    const uint4 *offs4 = (const uint4 *)(stage + XL_DATA + 1);
+    if (XS) {
+        tw = xl_tab[((size_t)xs * NT + T) * 32 + lane];
+        uint32_t nx[XL_ROWS];
+        xl_tile_load<0>(nx, Vt, tw, T, X0, lane, log2_n);
+        const int rows = (tw >> 8) & 63;
+#pragma unroll
+        for (int r = 0; r < XL_ROWS; r++)
+            if (r < 32 || r < rows) stage[r * XL_PITCH + lane] = nx[r];
+        stage[XL_DATA + 1 + lane] = (uint32_t)(((tw & 7) * XL_PITCH + lane) * 4);
+        __syncwarp();
+        xr_gather0(u, row, offs4);
+    } else {
+        bmine = B[(size_t)t * n + 32 * T + lane];
+        const uint32_t row0 = (uint32_t)(32 * T) << log2_n, c0 = (uint32_t)(X0 + lane);
+#pragma unroll
+        for (int k = 0; k < 32; k++) {
+            const int b = __shfl_sync(0xffffffffu, bmine, k);
+            const uint32_t off = row0 + ((uint32_t)k << log2_n) + ((c0 + (uint32_t)b) & (uint32_t)mx);
+            u[k] = *(const uint32_t *)(Vt + 4ull * off);
+        }
+    }
+    // pass 1: (M, D) of this tile
+    uint32_t lo = u[0];
+#pragma unroll
+    for (int k = 1; k + 1 < 32; k += 2) lo = __vimin3_u32(lo, u[k], u[k + 1]);
+    const bool blocked_any = min(lo, u[31]) == 0u;
+    {
+        uint32_t tt = VI_INF, wp = 0u, d = 0u;
+        if (up) SummaryLoop<true, SOFT>::run(u, tt, wp, d, w, s0, s1);
+        else SummaryLoop<false, SOFT>::run(u, tt, wp, d, w, s0, s1);
+        if (!SOFT) d = 32u * w;
+        sMD[T * 32 + lane] = make_uint2(__viaddmin_u32(tt, wp, 0x7fffffffu), blocked_any ? SX_D_CAP : d);
+    }
+    __syncthreads();
+    // ripple: the sections before this one, in travel order
+    uint32_t c = VI_INF;
+    if (up) { for (int p = 0; p < T; p++) { const uint2 md = sMD[p * 32 + lane]; c = __viaddmin_u32(c, md.y, md.x); } }
+    else { for (int p = NT - 1; p > T; p--) { const uint2 md = sMD[p * 32 + lane]; c = __viaddmin_u32(c, md.y, md.x); } }
+    // pass 2
+    uint32_t cm = 0, wp = 0u;
+    if (!fixed && tile_is_idle4(u, c)) { }
+    else if (up) RelaxLoop<true, SOFT>::run(u, c, wp, w, ct, s0, s1, cm);
+    else RelaxLoop<false, SOFT>::run(u, c, wp, w, ct, s0, s1, cm);
+    if (fixed == 1) cm = 0xffffffffu;                       // NHP_FLAG_FIXED_WORK: every vertex goes back
+    if (XS) {
+        const uint32_t lines = __ballot_sync(0xffffffffu, cm != 0u);
+        if (lines) {
+            xr_scatter0(u, row, offs4, cm);
+            __syncwarp();
+            xl_stage_store(stage, Vt, tw, T, X0, lane, log2_n, lines);
+        }
+    } else if (__any_sync(0xffffffffu, cm != 0u)) {
+        const uint32_t row0 = (uint32_t)(32 * T) << log2_n, c0 = (uint32_t)(X0 + lane);
+#pragma unroll
+        for (int k = 0; k < 32; k++) {
+            const int b = __shfl_sync(0xffffffffu, bmine, k);
+            const uint32_t off = row0 + ((uint32_t)k << log2_n) + ((c0 + (uint32_t)b) & (uint32_t)mx);
+            if ((cm >> k) & 1u) st_global(Vt, off, u[k]);
+        }
+    }
+}
+
 }  // namespace
 
 // SF or SB over the whole volume: one launch for the slices with I = 0 (tiles transposed through shared memory)
@@ -371,6 +524,15 @@ int launch_straight_tile(nhp_planner *p, int m)
     const dim3 gy(bands / warps, ny);
     const int fwd = (m == M_SF);
     const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : (p->w.flags & NHP_FLAG_NO_SHORTCUTS) ? 2 : 0;   // 1: no short cuts, store all; 2: no short cuts
+    // Sections (one warp per tile, all tiles of a band at once): small grids, or on request; at most 16 tiles per line
+    if (bands <= 16 && !(p->w.flags & NHP_FLAG_NO_SECTIONS) && (n <= 256 || (p->w.flags & NHP_FLAG_SECTIONS))) {
+        const size_t smx = sizeof(uint32_t) * (size_t)bands * (64 + XL_STAGE), smy = sizeof(uint32_t) * (size_t)bands * 64;
+#define NHP_SX(XS, SO, G, SM) straight_sect_kernel<XS, SO><<<G, bands * 32, SM, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, XS ? p->d_tlist : p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed)
+        { ProfScope px(p, 14); if (soft) NHP_SX(true, true, dim3(bands, nx), smx); else NHP_SX(true, false, dim3(bands, nx), smx); }
+        { ProfScope py(p, 15); if (soft) NHP_SX(false, true, dim3(bands, ny), smy); else NHP_SX(false, false, dim3(bands, ny), smy); }
+#undef NHP_SX
+        return 2;
+    }
     {
         const int xw = bands < XL_WARPS_V ? bands : XL_WARPS_V;
         const size_t smem = sizeof(uint32_t) * (size_t)xw * XL_STAGE;
@@ -396,5 +558,9 @@ int set_softlayout_attributes();               // softlayout.cu
 int set_kernel_attributes(nhp_planner *p)
 {
     (void)p;
+    const int sect_smem = 4 * 16 * (64 + XL_STAGE);
+    if (cudaFuncSetAttribute(straight_sect_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess ||
+        cudaFuncSetAttribute(straight_sect_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess)
+        return NHP_E_CUDA;
     return set_softlayout_attributes();
 }

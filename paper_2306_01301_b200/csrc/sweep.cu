@@ -292,6 +292,65 @@ __device__ __forceinline__ void checksum_add(unsigned long long &acc, uint32_t v
     asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(v), "r"(one));
 }
 
+// Soft costs: ONE chain per thread over its section of L = 32 vertices (the per-vertex weight already gives the integer and
+// the multiplier pipe independent work next to the chain, and a second chain's state does not fit the 64 registers of a
+// 512-thread tile).  The S bytes come from the tile-major copy of the soft volume (softlayout.cu): word j of a section holds
+// the bytes of its vertices 4 j .. 4 j + 3 for one curve, the 32 curves of the tile next to each other, so a warp reads one
+// 128-byte line per four vertices (sp points at this lane's word 0; the line of word j is 32 words further on).  The word
+// after the current one is fetched four vertices ahead.
+__device__ __forceinline__ uint32_t ld_s4(const uint32_t *p)
+{
+    uint32_t q;
+    asm volatile("ld.global.nc.u32 %0, [%1];" : "=r"(q) : "l"(p));
+    return q;
+}
+
+// The pointer plus (x >> 31) words.  Every value x this is used with is below 2^31, so nothing is added -- but the instruction
+// scheduler cannot know that, and the loads through the returned pointer (and the weight arithmetic that hangs on them) cannot
+// be hoisted above the point where x is known.  Without it the weights of a whole pass are formed during the pass before it
+// and spilled (the tile itself takes half the 64 registers).
+__device__ __forceinline__ const uint32_t *after_value(const uint32_t *p, uint32_t x)
+{
+    return p + (x >> 31);
+}
+
+template <int L, bool UP, bool CS, int S = 0>
+struct SoftLoop {
+    static constexpr int k = UP ? S : L - 1 - S;
+    static constexpr int knext = UP ? S + 4 : L - 1 - (S + 4);          // first vertex of the following word, in travel order
+    static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const uint32_t *sp, uint32_t len4, uint32_t &t, uint32_t &w, uint32_t &d,
+                                                   uint32_t q, uint32_t qn, uint32_t one)
+    {
+        if (S % 4 == 0) { q = qn; if (S + 4 < L) qn = ld_s4(sp + 32 * (knext >> 2)); }
+        const uint32_t u = col[k];
+        const uint32_t wk = nhp_soft_weight(len4, q, k & 3);
+        t = nhp_gate(nhp_arrive(t, w, u), u);
+        w = wk;
+        asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(d) : "r"(w), "r"(one));      // on the FMA pipe (IMAD with the parameter 1)
+        SoftLoop<L, UP, CS, S + 1>::summary(col, sp, len4, t, w, d, q, qn, one);
+    }
+    static __device__ __forceinline__ void apply(uint32_t (&col)[L], const uint32_t *sp, uint32_t len4, uint32_t ct, uint32_t &t, uint32_t &w, uint32_t q,
+                                                 uint32_t qn, unsigned long long &acc, uint32_t one)
+    {
+        if (S % 4 == 0) { q = qn; if (S + 4 < L) qn = ld_s4(sp + 32 * (knext >> 2)); }
+        const uint32_t u = col[k];
+        const uint32_t wk = nhp_soft_weight(len4, q, k & 3);
+        t = nhp_arrive(t, w, u);
+        col[k] = nhp_keep(t, ct, u);
+        if (CS) checksum_add(acc, col[k], one);
+        t = nhp_gate(t, u);
+        w = wk;
+        SoftLoop<L, UP, CS, S + 1>::apply(col, sp, len4, ct, t, w, q, qn, acc, one);
+    }
+};
+template <int L, bool UP, bool CS>
+struct SoftLoop<L, UP, CS, L> {
+    static __device__ __forceinline__ void summary(const uint32_t (&)[L], const uint32_t *, uint32_t, uint32_t &, uint32_t &, uint32_t &, uint32_t, uint32_t,
+                                                   uint32_t) {}
+    static __device__ __forceinline__ void apply(uint32_t (&)[L], const uint32_t *, uint32_t, uint32_t, uint32_t &, uint32_t &, uint32_t, uint32_t,
+                                                 unsigned long long &, uint32_t) {}
+};
+
 struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4 (soft)
 
 // One maneuver over the tile.  All values travel as a = v - ct (nhp_arrive): a summary M is the value arriving at
@@ -356,6 +415,35 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
     return true;
 }
 
+// The same maneuver with soft costs (single chain, see SoftLoop).  Short cut kept: all_blocked.
+template <int L, bool UP, bool CS_AFTER>
+__device__ __forceinline__ bool turn_maneuver_soft(uint32_t (&col)[L], const uint32_t *sp, TurnPass pass, bool blocked_any, bool all_blocked, uint2 *sMD,
+                                                   int sec, int S, int lane, unsigned long long &after, uint32_t one, uint32_t &t_last)
+{
+    if (all_blocked) {
+        const uint2 md = make_uint2(0x7fffffffu, D_CAP);
+        sMD[sec * 32 + lane] = md;
+        sMD[(sec + S) * 32 + lane] = md;
+        __syncthreads();
+        return false;
+    }
+    constexpr int k0 = UP ? 0 : L - 1;
+    const uint32_t len4 = pass.w;
+    uint32_t t = VI_INF, w = 0u, d = 0u;
+    const uint32_t *sa = after_value(sp, t_last);             // not before the previous maneuver's last chain value
+    SoftLoop<L, UP, false>::summary(col, sa, len4, t, w, d, 0u, ld_s4(sa + 32 * (k0 >> 2)), one);
+    const uint2 md = make_uint2(__viaddmin_u32(t, w, 0x7fffffffu), blocked_any ? D_CAP : d);
+    sMD[sec * 32 + lane] = md;
+    sMD[(sec + S) * 32 + lane] = md;
+    __syncthreads();
+    t = ripple_carry<UP>(sMD, sec, S, lane);
+    const uint32_t *sb = after_value(sp, t);                  // not before the carry is known
+    w = 0u;
+    SoftLoop<L, UP, CS_AFTER>::apply(col, sb, len4, pass.ct, t, w, 0u, ld_s4(sb + 32 * (k0 >> 2)), after, one);
+    t_last = t;
+    return true;
+}
+
 // Row addressing of a tile: so[t] = element index of the tile's first vertex in plane t (row base + first column).
 // A tile whose 32 columns never cross the seam i = N-1 -> 0 ("!wraps", CTA-uniform) addresses vertex (t, lane) as
 // (V + lane)[so[t]]: one IMAD.WIDE per vertex; otherwise the column is wrapped per lane (one add + one bit-select more).
@@ -415,9 +503,16 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         so[t] = (uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n) + c0);
         seam |= (c0 > mx - 31);
     }
-    SecW<SOFT> sw;
+    SecW<false> sw;
     sw.len = 0;
-    sw.sp = SOFT ? (const uint4 *)(Scurve + ((((size_t)yp << log2_n) + x0 + lane) * nt + sec * L)) : nullptr;
+    sw.sp = nullptr;
+    // tile-major soft volume (softlayout.cu): tile (yp, x0 / 32) = nt / 4 lines of 32 words; this section's words 8 sec .. 8 sec + 7
+    const uint32_t *sp = nullptr;
+    if (SOFT) {
+        sp = (const uint32_t *)Scurve + (((size_t)yp << (log2_n - 5)) + blockIdx.x) * ((size_t)nt * 8) + (size_t)sec * (L / 4) * 32;
+        if (lane < L / 4) asm volatile("prefetch.global.L1 [%0];" ::"l"(sp + lane * 32));       // the section's eight lines, needed after the tile
+        sp += lane;
+    }
     const bool wraps = __syncthreads_or(seam) != 0;
     uint32_t col[L];
     if (!wraps) tile_rows_load<L, false>(col, V, so + sec * L, lane, (uint32_t)mx);
@@ -446,11 +541,20 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         for (int k = 0; k < L; k++) lowest = __viaddmin_u32(col[k], 0xffffffffu, lowest);
         no_finite = __all_sync(0xffffffffu, lowest >= VI_INF - 1u);
     }
-    const bool ran_a = turn_maneuver<L, UP0, SOFT, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
-                                                                lane, after, one);
-    bool ran_last = ran_a;
-    if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, SOFT, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
-                                                                  sMD + 2 * S * 32, sec, S, lane, after, one);
+    bool ran_a, ran_last;
+    if constexpr (SOFT) {
+        const bool blocked_any = blocked_lo || blocked_hi;
+        uint32_t t_last = 0u;
+        ran_a = turn_maneuver_soft<L, UP0, NPASS == 1>(col, sp, pa, blocked_any, all_blocked, sMD, sec, S, lane, after, one, t_last);
+        ran_last = ran_a;
+        if (NPASS == 2) ran_last = turn_maneuver_soft<L, !UP0, true>(col, sp, pb, blocked_any, all_blocked, sMD + 2 * S * 32, sec, S, lane, after, one, t_last);
+    } else {
+        ran_a = turn_maneuver<L, UP0, false, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
+                                                         lane, after, one);
+        ran_last = ran_a;
+        if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, false, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
+                                                                       sMD + 2 * S * 32, sec, S, lane, after, one);
+    }
     if (!ran_last) {                                          // the "after" sum lives in the last apply pass: take it here if that pass did not run
         after = before;
         if (NPASS == 2 && ran_a) {
@@ -510,6 +614,51 @@ static int launch_straight(nhp_planner *p, int m)
     return k ? k : launch_maneuver_simple(p, m);
 }
 
+// Launches of one inner cycle of the tile kernels, in the paper's order with the two fusions: forward only: LF, SF, RF; otherwise
+// SF, RB+RF, SB, LB+(next cycle's LF).
+static int launch_inner_cycle(nhp_planner *p, int L, bool fwd_only)
+{
+    int launches = 0;
+    if (fwd_only) {
+        launches += launch_turn_tile(p, L, M_LF, -1);
+        launches += launch_straight(p, M_SF);
+        launches += launch_turn_tile(p, L, M_RF, -1);
+    } else {
+        launches += launch_straight(p, M_SF);
+        launches += launch_turn_tile(p, L, M_RB, M_RF);
+        launches += launch_straight(p, M_SB);
+        launches += launch_turn_tile(p, L, M_LB, M_LF);
+    }
+    return launches;
+}
+
+// Small grids are bound by launch overhead (30 launches of a few microseconds each at 64^3): the launches of one
+// inner cycle are captured once, at creation, into a CUDA graph and replayed.  Captured on a private stream (the caller's may
+// be the legacy default stream, which cannot be captured); every kernel argument is fixed at creation.
+int build_cycle_graph(nhp_planner *p)
+{
+    const int L = turn_tile_L(p);
+    if (L == 0 || (size_t)p->n * p->n * p->nt > ((size_t)1 << 26)) return NHP_OK;
+    cudaStream_t cap = nullptr, user = p->stream;
+    if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) return NHP_E_CUDA;
+    const bool was_profiling = p->profiling;
+    p->profiling = false;
+    p->stream = cap;
+    bool ok = cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    int kernels = 0;
+    if (ok) {
+        kernels = launch_inner_cycle(p, L, (p->w.flags & NHP_FLAG_FORWARD_ONLY) != 0);
+        ok = cudaStreamEndCapture(cap, &p->cycle_graph) == cudaSuccess && p->cycle_graph != nullptr;
+    }
+    p->stream = user;
+    p->profiling = was_profiling;
+    if (ok) ok = cudaGraphInstantiate(&p->cycle_exec, p->cycle_graph, 0) == cudaSuccess;
+    cudaStreamDestroy(cap);
+    if (!ok) { cudaGetLastError(); return NHP_E_CUDA; }
+    p->cycle_graph_kernels = kernels;
+    return NHP_OK;
+}
+
 // Cycle driver, PAPER.md:392 + l.475: LF, SF, RB, RF, SB, LB per cycle.  FORWARD_ONLY keeps LF, SF, RF.
 // With the tile kernel, RB+RF run as one launch and LB is fused with the LF of the NEXT cycle (same curve family,
 // adjacent in the sequence), so the order of operations on every vertex is exactly the paper's.
@@ -518,6 +667,11 @@ int launch_cycles(nhp_planner *p, int n_cycles)
     int launches = 0;
     const bool fwd_only = p->w.flags & NHP_FLAG_FORWARD_ONLY;
     const int L = turn_tile_L(p);
+    const bool graph = p->cycle_exec != nullptr && !p->profiling;
+    auto inner = [&]() {
+        if (graph && cudaGraphLaunch(p->cycle_exec, p->stream) == cudaSuccess) return p->cycle_graph_kernels;
+        return launch_inner_cycle(p, L, fwd_only);
+    };
     for (int c = 0; c < n_cycles; c++) {
         if (L == 0) {
             for (int m = 0; m < 6; m++) {
@@ -525,15 +679,16 @@ int launch_cycles(nhp_planner *p, int n_cycles)
                 launches += (m == M_SF || m == M_SB) ? launch_straight(p, m) : launch_maneuver_simple(p, m);
             }
         } else if (fwd_only) {
-            launches += launch_turn_tile(p, L, M_LF, -1);
-            launches += launch_straight(p, M_SF);
-            launches += launch_turn_tile(p, L, M_RF, -1);
+            launches += inner();
         } else {
             if (c == 0) launches += launch_turn_tile(p, L, M_LF, -1);
-            launches += launch_straight(p, M_SF);
-            launches += launch_turn_tile(p, L, M_RB, M_RF);
-            launches += launch_straight(p, M_SB);
-            launches += (c + 1 < n_cycles) ? launch_turn_tile(p, L, M_LB, M_LF) : launch_turn_tile(p, L, M_LB, -1);
+            if (c + 1 < n_cycles) launches += inner();
+            else {
+                launches += launch_straight(p, M_SF);
+                launches += launch_turn_tile(p, L, M_RB, M_RF);
+                launches += launch_straight(p, M_SB);
+                launches += launch_turn_tile(p, L, M_LB, -1);
+            }
         }
     }
     return launches;

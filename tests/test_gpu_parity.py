@@ -40,7 +40,8 @@ def small_scenes():
     ]
 
 
-@pytest.mark.parametrize("flags", [0, 4, 8, 16])     # tile kernels, thread-per-curve kernels, NHP_FLAG_FIXED_WORK, NHP_FLAG_NO_SHORTCUTS
+@pytest.mark.parametrize("flags", [0, 4, 8, 16, 64, 64 | 8])     # tile kernels (straight sweeps by Sections at these sizes), thread-per-curve kernels,
+                                                                  # NHP_FLAG_FIXED_WORK, NHP_FLAG_NO_SHORTCUTS, NHP_FLAG_NO_SECTIONS (streaming straight kernels), the same with fixed work
 def test_tables_render_sweeps_and_plans_match_the_oracle(mods, flags):
     oracle, nhp = mods
     for sc in small_scenes():
@@ -473,6 +474,34 @@ def test_errors_and_degenerate_cases(mods):
     with pytest.raises(nhp.NhpError) as e:
         nhp.Planner(9, 8, 80.0, sc.ct)                            # N_theta < 2 pi R
     assert e.value.code == -3
+
+
+def _sweeps_match(mods, sc, flags, n_cycles):
+    oracle, nhp = mods
+    o, fp = oracle_for(oracle, sc, threads=0)
+    p = nhp.Planner.from_scene(sc, flags=flags)
+    p.render_obstacles(sc.hard, sc.soft)
+    Cv, Sv = o.render(fp, sc.hard, sc.soft, method="runs")
+    assert (p.collision_numpy() == Cv).all()
+    p.run_nturn(sc.start, n_cycles)
+    got = p.cost_volume_numpy()
+    V = o.run(Cv, Sv, sc.start, n_cycles)
+    assert (got == V).all(), (sc.name, flags, int((got != V).sum()))
+    assert (V != INF).any()
+    p.close()
+
+
+def test_straight_sections_and_streaming_at_the_other_sizes(mods):
+    """The two forms of the straight sweeps (Sections, appendix D, default up to 256 cells; streaming kernels,
+    default from 512 cells) each at the sizes where they are not the default, and the extremes: one tile per line (N = 32),
+    sixteen sections per line (N = 512, hard and soft), 64 tiles per line (N = 2048)."""
+    oracle, nhp = mods
+    _sweeps_match(mods, scenes.random_scene(5, 6, 4, 21, n_cycles=2), 0, 2)                                  # N = 32: one section
+    _sweeps_match(mods, scenes.random_scene(5, 6, 4, 21, n_cycles=2), nhp.FLAG_NO_SECTIONS, 2)
+    _sweeps_match(mods, scenes.get_config(3), nhp.FLAG_SECTIONS, 3)                                          # N = 512: 16 sections
+    _sweeps_match(mods, scenes.get_config(4), nhp.FLAG_SECTIONS, 2)                                          # ... with soft costs
+    _sweeps_match(mods, scenes.get_config(3), nhp.FLAG_SECTIONS | nhp.FLAG_FIXED_WORK, 1)
+    _sweeps_match(mods, scenes.random_scene(11, 6, 8, 22, vehicle=(9, 4), n_rects=60, n_cycles=1), 0, 1)     # N = 2048: streaming
 
 
 def _full_config(mods, k, sample_render=20000):
