@@ -65,7 +65,7 @@ def measured_traffic(config, slot):
             for ln in f:
                 if ln.startswith("#") or not ln.strip():
                     continue
-                c, k, b, src = ln.strip().split(",")
+                c, k, b, src = ln.strip().split(",", 3)
                 if c == str(config) and k == slot:
                     return {"bytes_per_launch": int(b), "source": src}
     except OSError:

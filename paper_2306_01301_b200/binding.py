@@ -120,10 +120,13 @@ def query_sizes(log2_n, log2_ntheta, flags=0, max_footprint_radius=0, max_reach_
 class Planner:
     """One planner handle = one grid, one stream.  Method names follow the C ABI without the nhp_ prefix."""
 
+    GUARD_BYTE = 0xA5
+
     def __init__(self, log2_n, log2_ntheta, R, ct, dir_mult=(256,) * 6, cost_one_log2=10, flags=0, device="cuda:0",
-                 stream=None, max_footprint_radius=0, reach_levels=0):
+                 stream=None, max_footprint_radius=0, reach_levels=0, guard_bytes=0):
         """max_footprint_radius / reach_levels: the nhp_limits the workspace is sized for (0 = the library's defaults:
-        radius min(64, N/2 - 1), no reachability planner)."""
+        radius min(64, N/2 - 1), no reachability planner).  guard_bytes > 0 (a multiple of 256; test aid): every buffer
+        handed to the library sits between two guard bands of that many bytes, see guards_intact()."""
         import torch
         self._L = load_library()
         if not torch.cuda.is_available():
@@ -134,11 +137,23 @@ class Planner:
         self.shape = (self.nt, self.n, self.n)
         self.flags = flags
         sz = query_sizes(log2_n, log2_ntheta, flags, max_footprint_radius, reach_levels)
+        assert guard_bytes % 256 == 0
+        self._guarded = []
+
+        def buf(nbytes, dtype):
+            raw = torch.empty(nbytes + 2 * guard_bytes, dtype=torch.uint8, device=self.device)
+            if guard_bytes:
+                raw[:guard_bytes] = self.GUARD_BYTE
+                raw[guard_bytes + nbytes:] = self.GUARD_BYTE
+                self._guarded.append((raw, nbytes))
+            return raw[guard_bytes:guard_bytes + nbytes].view(dtype)
+
         with torch.cuda.device(self.device):
-            self.V = torch.empty(sz.V_bytes // 4, dtype=torch.int32, device=self.device)
-            self.C = torch.empty(sz.C_bytes // 4, dtype=torch.int32, device=self.device)
-            self.S = torch.empty(sz.S_bytes, dtype=torch.uint8, device=self.device) if sz.S_bytes else None
-            self.W = torch.empty(sz.workspace_bytes, dtype=torch.uint8, device=self.device)
+            self.V = buf(sz.V_bytes, torch.int32)
+            self.C = buf(sz.C_bytes, torch.int32)
+            self.S = buf(sz.S_bytes, torch.uint8) if sz.S_bytes else None
+            self.W = buf(sz.workspace_bytes, torch.uint8)
+            self._guard_bytes = guard_bytes
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             w = Weights((C.c_uint32 * 6)(*ct), (C.c_uint32 * 6)(*dir_mult), cost_one_log2, flags)
             b = Buffers(self.V.data_ptr(), self.C.data_ptr(), self.S.data_ptr() if self.S is not None else None, self.W.data_ptr())
@@ -149,6 +164,12 @@ class Planner:
         if rc:
             raise NhpError(rc, "planner_create")
         self._h = h
+
+    def guards_intact(self):
+        """True iff no byte of any guard band around V, C, S and the workspace has been written (needs guard_bytes > 0)."""
+        self.torch.cuda.synchronize(self.device)
+        g = self._guard_bytes
+        return all(bool((raw[:g] == self.GUARD_BYTE).all()) and bool((raw[g + n:] == self.GUARD_BYTE).all()) for raw, n in self._guarded)
 
     @classmethod
     def from_scene(cls, sc, flags=0, **kw):

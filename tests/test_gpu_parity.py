@@ -504,6 +504,35 @@ def test_straight_sections_and_streaming_at_the_other_sizes(mods):
     _sweeps_match(mods, scenes.random_scene(11, 6, 8, 22, vehicle=(9, 4), n_rects=60, n_cycles=1), 0, 1)     # N = 2048: streaming
 
 
+def test_no_write_outside_the_buffers_and_run_to_run_identical(mods):
+    """Stand-in for the memory / race checker (compute-sanitizer is closed on this pool, profiles/r02_sanitizer.md): every buffer
+    handed to the library lies between guard bands that must stay untouched through footprint, rendering, both planners, every
+    kernel variant and back-tracking; and the same plan run five times gives the same volume bit for bit (no two
+    threads of a maneuver kernel touch the same vertex, so nothing may depend on scheduling)."""
+    oracle, nhp = mods
+    for sc, flags in ((scenes.random_scene(6, 6, 8, 31, soft=True, reverse_mult=512, vehicle=(5, 2), n_rects=10), 0),
+                      (scenes.random_scene(6, 6, 8, 31, soft=True, reverse_mult=512, vehicle=(5, 2), n_rects=10), nhp.FLAG_NO_SECTIONS | nhp.FLAG_FIXED_WORK),
+                      (scenes.random_scene(5, 10, 6, 32, n_cycles=2), 0),                    # N_theta = 1024: 32 sections per turn tile
+                      (scenes.random_scene(8, 5, 4.5, 33, vehicle=(3, 2), n_rects=40, n_cycles=2), nhp.FLAG_SIMPLE_KERNELS),
+                      (scenes.random_scene(7, 6, 9, 34, flags=1, soft=True), nhp.FLAG_NO_SHORTCUTS),  # forward only
+                      (scenes.get_config(2), 0), (scenes.get_config(3), nhp.FLAG_SECTIONS)):
+        p = nhp.Planner.from_scene(sc, flags=flags, guard_bytes=1 << 16, reach_levels=4)
+        vols = []
+        for rep in range(5 if sc.n <= 256 else 2):
+            p.render_obstacles(sc.hard, sc.soft)
+            p.run_nturn(sc.start, sc.n_cycles)
+            vols.append(p.cost_volume().clone())
+            try:
+                p.extract_path(sc.goal)
+            except nhp.NhpError as e:
+                assert e.code == -5
+        assert all(bool((v == vols[0]).all()) for v in vols[1:]), sc.name
+        p.reach_run(sc.start, 4)
+        p.reach_count_numpy()
+        assert p.guards_intact(), (sc.name, flags)
+        p.close()
+
+
 def _full_config(mods, k, sample_render=20000):
     oracle, nhp = mods
     sc = scenes.get_config(k)
