@@ -115,6 +115,19 @@ def test_run_renderer_equals_brute_force(seed, vehicle, soft):
         assert c == Cb[t, j, i] and (Sb is None or s == Sb[t, j, i])
 
 
+def test_run_renderer_equals_brute_force_with_a_large_footprint():
+    """The vehicle of config 5 (44 x 20 cells: footprint radius 38, runs up to 44 cells long, i.e. every level of the sparse
+    tables of row maxima / prefix counts up to 2^5) on a small grid, whole volume against the plain O(N_R |box|) loop."""
+    for vehicle, seed in (((44, 20), 41),):
+        sc = scenes.random_scene(7, 4, 2.4, seed, vehicle=vehicle, n_rects=14, max_side=9, soft=True)
+        o = oracle.Oracle(sc.log2_n, sc.log2_nt, sc.R, sc.ct)
+        fp = oracle.Footprint(sc.mask, sc.ou, sc.ov)
+        Cb, Sb = o.render(fp, sc.hard, sc.soft, method="brute")
+        Cr, Sr = o.render(fp, sc.hard, sc.soft, method="runs")
+        assert (Cb == Cr).all() and (Sb == Sr).all()
+        assert 0 < Cb.mean() < 1
+
+
 def test_footprint_overhanging_the_seam_is_blocked():
     """PAPER.md:226 + DESIGN R13: image addressing is toroidal and the pixels a = 0, b = 0 are hard."""
     o = make()
