@@ -282,6 +282,30 @@ __device__ __forceinline__ uint32_t ripple_carry(const uint2 *sMD, int sec, int 
     return c;
 }
 
+// The same walk with the loads four sections ahead of the fold (the soft kernel has the registers for it at this point; in the hard
+// kernel this form measured slower: 139 -> 144 us per pair)
+template <bool UP>
+__device__ __forceinline__ uint32_t ripple_carry_ahead(const uint2 *sMD, int sec, int S, int lane)
+{
+    const uint2 *q = sMD + (UP ? sec : sec + S) * 32 + lane;
+    constexpr int step = UP ? 32 : -32;
+    uint32_t c = q->x;
+    // four (M, D) pairs are fetched while the four before them are folded: the dependent chain is the DPX ops, not the loads
+    uint2 cur[4];
+#pragma unroll
+    for (int i = 0; i < 4; i++) cur[i] = (1 + i < S) ? q[(1 + i) * step] : make_uint2(0xffffffffu, 0u);
+    for (int r = 1; r < S; r += 4) {
+        uint2 nxt[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) nxt[i] = (r + 4 + i < S) ? q[(r + 4 + i) * step] : make_uint2(0xffffffffu, 0u);
+#pragma unroll
+        for (int i = 0; i < 4; i++) c = __viaddmin_u32(c, cur[i].y, cur[i].x);      // padding (M = 2^32 - 1, D = 0) leaves c as it is
+#pragma unroll
+        for (int i = 0; i < 4; i++) cur[i] = nxt[i];
+    }
+    return c;
+}
+
 // Exact change detection: the 64-bit sums of a thread's 32 vertices before and after the passes differ iff a vertex
 // improved (values only decrease).  The additions are IMAD.WIDE on the FMA pipe; the "after" sum sits INSIDE the last
 // apply loop, in the issue slots the min/max pipe leaves free (it takes one warp instruction every other cycle); the
@@ -436,7 +460,7 @@ __device__ __forceinline__ bool turn_maneuver_soft(uint32_t (&col)[L], const uin
     sMD[sec * 32 + lane] = md;
     sMD[(sec + S) * 32 + lane] = md;
     __syncthreads();
-    t = ripple_carry<UP>(sMD, sec, S, lane);
+    t = ripple_carry_ahead<UP>(sMD, sec, S, lane);
     const uint32_t *sb = after_value(sp, t);                  // not before the carry is known
     w = 0u;
     SoftLoop<L, UP, CS_AFTER>::apply(col, sb, len4, pass.ct, t, w, 0u, ld_s4(sb + 32 * (k0 >> 2)), after, one);
@@ -496,12 +520,14 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     uint2 *sMD = (uint2 *)(so + nt);                          // [2][2 S][32] (M, D) of every section (twice), one set per maneuver
     const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
-    int seam = 0;
-    for (int t = threadIdx.x; t < nt; t += blockDim.x) {
+    // every warp fills in the rows of its own 32 planes: no CTA-wide barrier stands between the start of a tile and its loads
+    int seam;
+    {
+        const int t = sec * L + lane;
         const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];     // eq (18)
         const int c0 = (x0 + ba) & mx;
         so[t] = (uint32_t)((((t << log2_n) + ((yp + bb) & mx)) << log2_n) + c0);
-        seam |= (c0 > mx - 31);
+        seam = (c0 > mx - 31);
     }
     SecW<false> sw;
     sw.len = 0;
@@ -513,7 +539,8 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         if (lane < L / 4) asm volatile("prefetch.global.L1 [%0];" ::"l"(sp + lane * 32));       // the section's eight lines, needed after the tile
         sp += lane;
     }
-    const bool wraps = __syncthreads_or(seam) != 0;
+    const bool wraps = __any_sync(0xffffffffu, seam) != 0;      // warp-uniform
+    __syncwarp();
     uint32_t col[L];
     if (!wraps) tile_rows_load<L, false>(col, V, so + sec * L, lane, (uint32_t)mx);
     else tile_rows_load<L, true>(col, V, so + sec * L, lane, (uint32_t)mx);
