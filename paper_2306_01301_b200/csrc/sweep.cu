@@ -343,15 +343,16 @@ struct SoftLoop {
     static constexpr int k = UP ? S : L - 1 - S;
     static constexpr int knext = UP ? S + 4 : L - 1 - (S + 4);          // first vertex of the following word, in travel order
     static __device__ __forceinline__ void summary(const uint32_t (&col)[L], const uint32_t *sp, uint32_t len4, uint32_t &t, uint32_t &w, uint32_t &d,
-                                                   uint32_t q, uint32_t qn, uint32_t one)
+                                                   uint32_t q, uint32_t qn, unsigned long long &acc, uint32_t one)
     {
         if (S % 4 == 0) { q = qn; if (S + 4 < L) qn = ld_s4(sp + 32 * (knext >> 2)); }
         const uint32_t u = col[k];
+        if (CS) checksum_add(acc, u, one);
         const uint32_t wk = nhp_soft_weight(len4, q, k & 3);
         t = nhp_gate(nhp_arrive(t, w, u), u);
         w = wk;
         asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(d) : "r"(w), "r"(one));      // on the FMA pipe (IMAD with the parameter 1)
-        SoftLoop<L, UP, CS, S + 1>::summary(col, sp, len4, t, w, d, q, qn, one);
+        SoftLoop<L, UP, CS, S + 1>::summary(col, sp, len4, t, w, d, q, qn, acc, one);
     }
     static __device__ __forceinline__ void apply(uint32_t (&col)[L], const uint32_t *sp, uint32_t len4, uint32_t ct, uint32_t &t, uint32_t &w, uint32_t q,
                                                  uint32_t qn, unsigned long long &acc, uint32_t one)
@@ -370,7 +371,7 @@ struct SoftLoop {
 template <int L, bool UP, bool CS>
 struct SoftLoop<L, UP, CS, L> {
     static __device__ __forceinline__ void summary(const uint32_t (&)[L], const uint32_t *, uint32_t, uint32_t &, uint32_t &, uint32_t &, uint32_t, uint32_t,
-                                                   uint32_t) {}
+                                                   unsigned long long &, uint32_t) {}
     static __device__ __forceinline__ void apply(uint32_t (&)[L], const uint32_t *, uint32_t, uint32_t, uint32_t &, uint32_t &, uint32_t, uint32_t,
                                                  unsigned long long &, uint32_t) {}
 };
@@ -387,10 +388,10 @@ struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4
 //   no_finite     (hard costs only) no vertex of the warp holds a finite value yet: the section generates nothing
 //                 (M = infinity, D as always), and if no finite value arrives either, the apply pass has nothing to do
 // Returns true iff the apply pass ran (the vertices may have changed).
-template <int L, bool UP, bool SOFT, bool CS_AFTER>
+template <int L, bool UP, bool SOFT, bool CS_AFTER, bool CS_BEFORE>
 __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
                                               bool all_blocked, bool none_blocked, bool &no_finite, uint2 *sMD, int sec, int S, int lane,
-                                              unsigned long long &after, uint32_t one)
+                                              unsigned long long &after, unsigned long long &before, uint32_t one)
 {
     if (all_blocked) {
         const uint2 md = make_uint2(0x7fffffffu, D_CAP);
@@ -409,6 +410,10 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
         uint32_t ta = ripple_carry<UP>(sMD, sec, S, lane);
         if (__all_sync(0xffffffffu, ta >= VI_INF)) return false;                 // nothing arrives: nothing changes
         // something arrives: the ordinary apply pass (M of H0 is infinite, so the carry into H1 is ta + D(H0))
+        // (no summary pass has run on this tile yet -- neither this maneuver's nor, in a pair, the one before: it would have cleared
+        // no_finite -- so the "before" sum of the change detection is still to be taken)
+#pragma unroll
+        for (int k = 0; k < L; k++) checksum_add(before, col[k], one);
         uint32_t tb = __viaddmin_u32(ta, ia ? D_CAP : dh, 0x7fffffffu), wa = pass.w, wb = pass.w;
         sw.len = pass.w;
         SecLoop<L, UP, SOFT, CS_AFTER, true>::apply(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), pass.ct, ta, wa, tb, wb, after, one);
@@ -418,9 +423,8 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
     const bool ia = UP ? blocked_lo : blocked_hi, ib = UP ? blocked_hi : blocked_lo;     // H0, H1 in travel order
     sw.len = pass.w;
     uint32_t ta = VI_INF, tb = VI_INF, wa = SOFT ? 0u : pass.w, wb = wa, da = 0, db = 0;
-    unsigned long long unused = 0;
-    if (none_blocked) SecLoop<L, UP, SOFT, false, false>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, unused, one);
-    else SecLoop<L, UP, SOFT, false, true>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, unused, one);
+    if (none_blocked) SecLoop<L, UP, SOFT, CS_BEFORE, false>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, before, one);
+    else SecLoop<L, UP, SOFT, CS_BEFORE, true>::summary(col, sw, make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0), ta, wa, da, tb, wb, db, before, one);
     if (!SOFT) da = db = (uint32_t)(L / 2) * pass.w;
     const uint32_t ma = __viaddmin_u32(ta, wa, 0x7fffffffu), mb = __viaddmin_u32(tb, wb, 0x7fffffffu);
     const uint32_t Da = ia ? D_CAP : da;
@@ -440,9 +444,10 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
 }
 
 // The same maneuver with soft costs (single chain, see SoftLoop).  Short cut kept: all_blocked.
-template <int L, bool UP, bool CS_AFTER>
+template <int L, bool UP, bool CS_AFTER, bool CS_BEFORE>
 __device__ __forceinline__ bool turn_maneuver_soft(uint32_t (&col)[L], const uint32_t *sp, TurnPass pass, bool blocked_any, bool all_blocked, uint2 *sMD,
-                                                   int sec, int S, int lane, unsigned long long &after, uint32_t one, uint32_t &t_last)
+                                                   int sec, int S, int lane, unsigned long long &after, unsigned long long &before, uint32_t one,
+                                                   uint32_t &t_last)
 {
     if (all_blocked) {
         const uint2 md = make_uint2(0x7fffffffu, D_CAP);
@@ -455,7 +460,7 @@ __device__ __forceinline__ bool turn_maneuver_soft(uint32_t (&col)[L], const uin
     const uint32_t len4 = pass.w;
     uint32_t t = VI_INF, w = 0u, d = 0u;
     const uint32_t *sa = after_value(sp, t_last);             // not before the previous maneuver's last chain value
-    SoftLoop<L, UP, false>::summary(col, sa, len4, t, w, d, 0u, ld_s4(sa + 32 * (k0 >> 2)), one);
+    SoftLoop<L, UP, CS_BEFORE>::summary(col, sa, len4, t, w, d, 0u, ld_s4(sa + 32 * (k0 >> 2)), before, one);
     const uint2 md = make_uint2(__viaddmin_u32(t, w, 0x7fffffffu), blocked_any ? D_CAP : d);
     sMD[sec * 32 + lane] = md;
     sMD[(sec + S) * 32 + lane] = md;
@@ -552,12 +557,14 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         hi = __vimin3_u32(hi, col[L / 2 + k], col[L / 2 + k + 1]);
     }
     const bool blocked_lo = min(lo, col[L / 2 - 1]) == 0u, blocked_hi = min(hi, col[L - 1]) == 0u;
+    // change detection: `before` is summed inside the first summary pass, `after` inside the last apply pass (checksum_add)
     unsigned long long before = 0, after = 0;
+    // `fixed` (NHP_FLAG_FIXED_WORK / NHP_FLAG_NO_SHORTCUTS) switches the three short cuts off; fixed == 1 also stores every row: the same
+    // instructions and bytes whatever the volume holds
+    uint32_t top = col[0];
 #pragma unroll
-    for (int k = 0; k < L; k++) checksum_add(before, col[k], one);
-    // `fixed` (NHP_FLAG_FIXED_WORK) switches the three short cuts off and stores every row: the same instructions and
-    // bytes whatever the volume holds
-    const bool all_blocked = !fixed && __all_sync(0xffffffffu, before == 0ull);
+    for (int k = 1; k + 1 < L; k += 2) top = __vimax3_u32(top, col[k], col[k + 1]);
+    const bool all_blocked = !fixed && __all_sync(0xffffffffu, max(top, col[L - 1]) == 0u);
     // (soft kernels keep one chain variant: a second copy of their loops costs registers they do not have)
     const bool none_blocked = !SOFT && !fixed && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
     // "no finite value in this warp yet": min over (v - 1) with wrap-around (blocked 0 -> 2^32 - 1, unreached -> 2^30)
@@ -572,15 +579,15 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     if constexpr (SOFT) {
         const bool blocked_any = blocked_lo || blocked_hi;
         uint32_t t_last = 0u;
-        ran_a = turn_maneuver_soft<L, UP0, NPASS == 1>(col, sp, pa, blocked_any, all_blocked, sMD, sec, S, lane, after, one, t_last);
+        ran_a = turn_maneuver_soft<L, UP0, NPASS == 1, true>(col, sp, pa, blocked_any, all_blocked, sMD, sec, S, lane, after, before, one, t_last);
         ran_last = ran_a;
-        if (NPASS == 2) ran_last = turn_maneuver_soft<L, !UP0, true>(col, sp, pb, blocked_any, all_blocked, sMD + 2 * S * 32, sec, S, lane, after, one, t_last);
+        if (NPASS == 2) ran_last = turn_maneuver_soft<L, !UP0, true, false>(col, sp, pb, blocked_any, all_blocked, sMD + 2 * S * 32, sec, S, lane, after, before, one, t_last);
     } else {
-        ran_a = turn_maneuver<L, UP0, false, NPASS == 1>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
-                                                         lane, after, one);
+        ran_a = turn_maneuver<L, UP0, false, NPASS == 1, true>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
+                                                               lane, after, before, one);
         ran_last = ran_a;
-        if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, false, true>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
-                                                                       sMD + 2 * S * 32, sec, S, lane, after, one);
+        if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, false, true, false>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
+                                                                              sMD + 2 * S * 32, sec, S, lane, after, before, one);
     }
     if (!ran_last) {                                          // the "after" sum lives in the last apply pass: take it here if that pass did not run
         after = before;
