@@ -138,7 +138,7 @@ def pick_goal(p, sc, torch):
     return tuple(cands[best]) if vals[best] != 0xFFFFFFFF else tuple(sc.start)
 
 
-SWEEP_SLOTS = ("turn_pair", "LF", "RB", "RF", "LB", "straight_xrows", "straight_rows")
+SWEEP_SLOTS = ("turn_pair", "LF", "RB", "RF", "LB", "straight_xrows", "straight_rows", "straight_sect")
 
 
 class PlanBench:

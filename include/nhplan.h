@@ -299,8 +299,9 @@ long long nhp_launch_count(const nhp_planner *p);
  *   slot 12     distance transform + soft-image synthesis (nhp_render_obstacles_dt)
  *   slot 13     one level of the reachability planner (all its launches: copy, six sweeps, transpositions)
  *   slot 14     the I = 0 ("x-rows") kernel of a straight maneuver alone, slot 15 its I = 1 ("rows") kernel alone: both are
- *               NESTED inside the SF / SB pair of slots 1 and 4 (do not add them to a sum over the slots) */
-#define NHP_KERNEL_SLOTS 16
+ *               NESTED inside the SF / SB pair of slots 1 and 4 (do not add them to a sum over the slots)
+ *   slot 16     a straight maneuver in its Sections form (one launch for both slice groups), nested in the same way */
+#define NHP_KERNEL_SLOTS 17
 int nhp_set_profiling(nhp_planner *p, int enable);
 int nhp_kernel_times(nhp_planner *p, double *ms_sum, long long *launches, int reset);
 /* Launches that ran untimed since creation because the event pool was exhausted (0 in any sane use). */

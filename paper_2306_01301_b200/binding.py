@@ -22,10 +22,10 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu")
-KERNEL_SLOTS = 16
+KERNEL_SLOTS = 17
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
-                     "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows")
-NESTED_SLOTS = ("straight_xrows", "straight_rows")        # bracketed inside SF / SB: not part of a sum over the slots
+                     "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows", "straight_sect")
+NESTED_SLOTS = ("straight_xrows", "straight_rows", "straight_sect")        # bracketed inside SF / SB: not part of a sum over the slots
 
 
 class Weights(C.Structure):

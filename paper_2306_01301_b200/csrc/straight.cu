@@ -419,15 +419,16 @@ struct SummaryLoop<UP, SOFT, 32> {
     static __device__ __forceinline__ void run(const uint32_t *, uint32_t &, uint32_t &, uint32_t &, uint32_t, const uint4 &, const uint4 &) {}
 };
 
-template <bool XS, bool SOFT>
+template <bool SOFT>
 __global__ void __launch_bounds__(512) straight_sect_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline, const int16_t *__restrict__ B,
                                                             const uint32_t *__restrict__ xl_tab, const uint8_t *__restrict__ IJ,
-                                                            const int16_t *__restrict__ tlist, const uint32_t *__restrict__ lenq, uint32_t ct,
+                                                            const int16_t *__restrict__ tlist, int n_xslices, const uint32_t *__restrict__ lenq, uint32_t ct,
                                                             int log2_n, int is_forward, int fixed)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int n = 1 << log2_n, mx = n - 1, NT = n >> 5;
     const int xs = blockIdx.y, t = tlist[xs];
+    const bool XS = xs < n_xslices;                                             // the list holds the slices with I = 0 first (block-uniform)
     const int lane = threadIdx.x & 31, T = threadIdx.x >> 5;                    // warp = tile T of the band
     const int X0 = blockIdx.x << 5;
     const bool up = (is_forward == ((IJ[t] >> 1) & 1));                         // eq (24)
@@ -526,11 +527,11 @@ int launch_straight_tile(nhp_planner *p, int m)
     const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : (p->w.flags & NHP_FLAG_NO_SHORTCUTS) ? 2 : 0;   // 1: no short cuts, store all; 2: no short cuts
     // Sections (one warp per tile, all tiles of a band at once): small grids, or on request; at most 16 tiles per line
     if (bands <= 16 && !(p->w.flags & NHP_FLAG_NO_SECTIONS) && (n <= 256 || (p->w.flags & NHP_FLAG_SECTIONS))) {
-        const size_t smx = sizeof(uint32_t) * (size_t)bands * (64 + XL_STAGE), smy = sizeof(uint32_t) * (size_t)bands * 64;
-#define NHP_SX(XS, SO, G, SM) straight_sect_kernel<XS, SO><<<G, bands * 32, SM, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, XS ? p->d_tlist : p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed)
-        { ProfScope px(p, 14); if (soft) NHP_SX(true, true, dim3(bands, nx), smx); else NHP_SX(true, false, dim3(bands, nx), smx); }
-        { ProfScope py(p, 15); if (soft) NHP_SX(false, true, dim3(bands, ny), smy); else NHP_SX(false, false, dim3(bands, ny), smy); }
-#undef NHP_SX
+        const size_t smx = sizeof(uint32_t) * (size_t)bands * (64 + XL_STAGE);
+        ProfScope ps(p, 16);                                     // both slice groups in ONE launch (the block index tells which)
+        if (soft) straight_sect_kernel<true><<<dim3(bands, nt), bands * 32, smx, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, p->d_tlist, nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        else straight_sect_kernel<false><<<dim3(bands, nt), bands * 32, smx, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, p->d_tlist, nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        return 1;
         return 2;
     }
     {
@@ -559,8 +560,8 @@ int set_kernel_attributes(nhp_planner *p)
 {
     (void)p;
     const int sect_smem = 4 * 16 * (64 + XL_STAGE);
-    if (cudaFuncSetAttribute(straight_sect_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess ||
-        cudaFuncSetAttribute(straight_sect_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess)
+    if (cudaFuncSetAttribute(straight_sect_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess ||
+        cudaFuncSetAttribute(straight_sect_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sect_smem) != cudaSuccess)
         return NHP_E_CUDA;
     return set_softlayout_attributes();
 }
