@@ -47,6 +47,8 @@ def parse_args():
                     help="time the reachability (bit-vector) planner of appendix C instead: render + N_T levels + back-track")
     ap.add_argument("--fixed-work", action="store_true", help="NHP_FLAG_FIXED_WORK: data-dependent short cuts off (PAPER.md:565)")
     ap.add_argument("--no-shortcuts", action="store_true", help="NHP_FLAG_NO_SHORTCUTS: every warp runs every pass; stores still only where a value improved")
+    ap.add_argument("--sections", action="store_true", help="NHP_FLAG_SECTIONS: straight sweeps by Sections (appendix D) also at 512 cells per side")
+    ap.add_argument("--no-sections", action="store_true", help="NHP_FLAG_NO_SECTIONS: streaming straight kernels also on small grids")
     ap.add_argument("--no-extra", action="store_true", help="skip the fixed-work pass and the configs 4 / 5 side runs")
     ap.add_argument("--dt-on-device", action="store_true",
                     help="soft configs: distance transform + soft image on the GPU (nhp_render_obstacles_dt) instead of the harness image")
@@ -298,7 +300,7 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank)
     sc = scenes.CONFIGS[args.config](replicas.replica_seed(args.config, rank))
     n_cycles = args.cycles or sc.n_cycles
-    flags = (nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0) | (nhp.FLAG_FIXED_WORK if args.fixed_work else 0) | (nhp.FLAG_NO_SHORTCUTS if args.no_shortcuts else 0)
+    flags = (nhp.FLAG_SIMPLE_KERNELS if args.simple_kernels else 0) | (nhp.FLAG_FIXED_WORK if args.fixed_work else 0) | (nhp.FLAG_NO_SHORTCUTS if args.no_shortcuts else 0) | (nhp.FLAG_SECTIONS if args.sections else 0) | (nhp.FLAG_NO_SECTIONS if args.no_sections else 0)
     b = PlanBench(nhp, torch, replicas, sc, n_cycles, dev, flags=flags, reach=args.reach, dt_on_device=args.dt_on_device)
     p, n_r, updates_per_plan, dt_dev = b.p, b.n_r, b.updates_per_plan, b.dt_dev
     b.warm_up(args.warmup)

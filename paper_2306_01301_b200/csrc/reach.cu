@@ -320,9 +320,9 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
     const int trows = n / 32 < 8 ? n / 32 : 8;                  // 32 x 32 blocks per CTA of the transposition
     const dim3 tgrid(nw, n / 32 / trows, nx > 0 ? nx : 1), tblk(32, trows);
     // sweeps: 16 planes (rows) per thread, as many words of curves per CTA as fit 512 threads (sections of different words
-    // do not talk to each other); 32 planes per thread only when a curve has more than 512 x 16 of them
+    // do not talk to each other); a curve has at most 4096 planes / rows (nhp_planner_create), i.e. at most 256 sections
     auto geom = [&](int len, int &PL, dim3 &blk, int &wgrid, size_t &smem, int table) {
-        PL = (len / 16 <= 512) ? 16 : 32;
+        PL = 16;
         const int S = len / PL;
         int wx = 512 / S; if (wx > nw) wx = nw; if (wx < 1) wx = 1;
         blk = dim3(wx, S); wgrid = nw / wx;
@@ -341,24 +341,17 @@ int launch_reach_run(nhp_planner *p, int si, int sj, int st, int n_levels, int *
         uint32_t *Lout = p->r_levels + (size_t)(m + 1) * W;
         cudaMemcpyAsync(Lout, Lin, sizeof(uint32_t) * W, cudaMemcpyDeviceToDevice, p->stream);
         // turn maneuvers, eq (18): LEFT (beta0, beta3), RIGHT (beta2, beta1); LF, RB travel Theta+, LB, RF Theta- (eqs (25)-(28))
-        if (PLn == 16) {
-            reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3, 1, !fwd_only);   // LF (+ LB)
-            reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1, !fwd_only, 1);   // RF (+ RB)
-        } else {
-            reach_turn2_kernel<32><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3, 1, !fwd_only);
-            reach_turn2_kernel<32><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1, !fwd_only, 1);
-        }
+        reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 0, 3, 1, !fwd_only);   // LF (+ LB)
+        reach_turn2_kernel<16><<<dim3(n, tw), tblk2, t2smem, p->stream>>>(Lout, Lin, p->C, p->d_beta, p->log2_n, nt, 2, 1, !fwd_only, 1);   // RF (+ RB)
         k += 3;
         if (ny > 0) {
-            if (PLr == 16) reach_rows2_kernel<16><<<dim3(ny, rw), rblk2, r2smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, !fwd_only);
-            else reach_rows2_kernel<32><<<dim3(ny, rw), rblk2, r2smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, !fwd_only);
+            reach_rows2_kernel<16><<<dim3(ny, rw), rblk2, r2smem, p->stream>>>(Lout, Lin, p->C, p->d_B, p->d_IJ, p->d_tlist + nx, p->log2_n, !fwd_only);
             k += 1;
         }
         if (nx > 0) {
             reach_transpose_kernel<false><<<tgrid, tblk, 0, p->stream>>>(p->r_Lt, Lin, p->d_tlist, p->log2_n);
             cudaMemsetAsync(p->r_Gt, 0, sizeof(uint32_t) * W, p->stream);
-            if (PLr == 16) reach_rows2_kernel<16><<<dim3(nx, rw), rblk2, r2smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, !fwd_only);
-            else reach_rows2_kernel<32><<<dim3(nx, rw), rblk2, r2smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, !fwd_only);
+            reach_rows2_kernel<16><<<dim3(nx, rw), rblk2, r2smem, p->stream>>>(p->r_Gt, p->r_Lt, p->r_Ct, p->d_B, p->d_IJ, p->d_tlist, p->log2_n, !fwd_only);
             reach_transpose_kernel<true><<<tgrid, tblk, 0, p->stream>>>(Lout, p->r_Gt, p->d_tlist, p->log2_n);
             k += 4;
         }
