@@ -391,13 +391,16 @@ struct TurnPass { uint32_t w, ct; };      // w: edge weight (hard) or len_q << 4
 template <int L, bool UP, bool SOFT, bool CS_AFTER, bool CS_BEFORE>
 __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw, TurnPass pass, bool blocked_lo, bool blocked_hi,
                                               bool all_blocked, bool none_blocked, bool &no_finite, uint2 *sMD, int sec, int S, int lane,
-                                              unsigned long long &after, unsigned long long &before, uint32_t one)
+                                              unsigned long long &after, unsigned long long &before, uint32_t one, bool &tile_idle)
 {
+    // The barrier of a maneuver also tells whether EVERY section of the tile is in one of the two "hands on nothing" states: then
+    // nothing can arrive anywhere, the ring need not be walked, and (the tile being unchanged) the same holds for the maneuver
+    // that follows in a pair (tile_idle, CTA-uniform)
     if (all_blocked) {
         const uint2 md = make_uint2(0x7fffffffu, D_CAP);
         sMD[sec * 32 + lane] = md;
         sMD[(sec + S) * 32 + lane] = md;
-        __syncthreads();
+        tile_idle = __syncthreads_and(1) != 0;
         return false;
     }
     if (!SOFT && no_finite) {
@@ -406,7 +409,8 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
         const uint2 md = make_uint2(0x7fffffffu, (ia || ib) ? D_CAP : 2 * dh);
         sMD[sec * 32 + lane] = md;
         sMD[(sec + S) * 32 + lane] = md;
-        __syncthreads();
+        tile_idle = __syncthreads_and(1) != 0;
+        if (tile_idle) return false;
         uint32_t ta = ripple_carry<UP>(sMD, sec, S, lane);
         if (__all_sync(0xffffffffu, ta >= VI_INF)) return false;                 // nothing arrives: nothing changes
         // something arrives: the ordinary apply pass (M of H0 is infinite, so the carry into H1 is ta + D(H0))
@@ -432,7 +436,7 @@ __device__ __forceinline__ bool turn_maneuver(uint32_t (&col)[L], SecW<SOFT> &sw
     const uint2 md = make_uint2(__viaddmin_u32(ma, ib ? D_CAP : db, mb), (ia || ib) ? D_CAP : da + db);
     sMD[sec * 32 + lane] = md;
     sMD[(sec + S) * 32 + lane] = md;
-    __syncthreads();
+    tile_idle = __syncthreads_and(0) != 0;                    // (0: this section may hand something on)
     ta = ripple_carry<UP>(sMD, sec, S, lane);                 // carry into H0
     tb = __viaddmin_u32(ta, Da, ma);                          // carry into H1: through H0, or from inside it
     // opaque copy of the weight: otherwise the per-vertex values of the summary pass are kept alive for the apply pass
@@ -575,19 +579,21 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
         for (int k = 0; k < L; k++) lowest = __viaddmin_u32(col[k], 0xffffffffu, lowest);
         no_finite = __all_sync(0xffffffffu, lowest >= VI_INF - 1u);
     }
-    bool ran_a, ran_last;
+    bool ran_a, ran_last, tile_idle = false;
     if constexpr (SOFT) {
         const bool blocked_any = blocked_lo || blocked_hi;
         uint32_t t_last = 0u;
         ran_a = turn_maneuver_soft<L, UP0, NPASS == 1, true>(col, sp, pa, blocked_any, all_blocked, sMD, sec, S, lane, after, before, one, t_last);
         ran_last = ran_a;
-        if (NPASS == 2) ran_last = turn_maneuver_soft<L, !UP0, true, false>(col, sp, pb, blocked_any, all_blocked, sMD + 2 * S * 32, sec, S, lane, after, before, one, t_last);
+        if (NPASS == 2)
+            ran_last = turn_maneuver_soft<L, !UP0, true, false>(col, sp, pb, blocked_any, all_blocked, sMD + 2 * S * 32, sec, S, lane, after, before, one, t_last);
     } else {
         ran_a = turn_maneuver<L, UP0, false, NPASS == 1, true>(col, sw, pa, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite, sMD, sec, S,
-                                                               lane, after, before, one);
+                                                               lane, after, before, one, tile_idle);
         ran_last = ran_a;
-        if (NPASS == 2) ran_last = turn_maneuver<L, !UP0, false, true, false>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
-                                                                              sMD + 2 * S * 32, sec, S, lane, after, before, one);
+        if (NPASS == 2 && !tile_idle)
+            ran_last = turn_maneuver<L, !UP0, false, true, false>(col, sw, pb, blocked_lo, blocked_hi, all_blocked, none_blocked, no_finite,
+                                                                  sMD + 2 * S * 32, sec, S, lane, after, before, one, tile_idle);
     }
     if (!ran_last) {                                          // the "after" sum lives in the last apply pass: take it here if that pass did not run
         after = before;
