@@ -314,6 +314,13 @@ long long nhp_prof_dropped(const nhp_planner *p);
  * Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_CUDA. */
 int nhp_microbench_alu(nhp_planner *p, int chains, double *lane_ops_per_s, int *sms);
 
+/* Read probe behind the roofline discussion: reads the whole value volume V once, nothing else, in the
+ * access pattern of one of the sweep kernels -- 0: linear 4 KB chunks, 1: straight_rows_kernel (a warp walks a band: 32 rows of
+ * 128 bytes per tile), 2: straight_xl_kernel (tiles follow each other along the rows), 3: turn_tile_kernel (one CTA per tile of 32
+ * curves, warp s reads planes 32 s .. 32 s + 31) -- on the handle's stream, timed with CUDA events, and returns bytes per second.
+ * V is not modified (its content does not matter).  Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_CUDA. */
+int nhp_microbench_read(nhp_planner *p, int pattern, double *bytes_per_s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -21,7 +21,7 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_render_vehicle_footprint", "nhp_set_box", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
-           "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu")
+           "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu", "nhp_microbench_read")
 KERNEL_SLOTS = 17
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
                      "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows", "straight_sect")
@@ -104,6 +104,7 @@ def load_library():
         L.nhp_set_profiling.argtypes = [C.c_void_p, C.c_int]
         L.nhp_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
         L.nhp_microbench_alu.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+        L.nhp_microbench_read.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -334,6 +335,12 @@ class Planner:
         ops, sms = C.c_double(0), C.c_int(0)
         self._check(self._L.nhp_microbench_alu(self._h, int(chains), C.byref(ops), C.byref(sms)), "microbench_alu")
         return ops.value, sms.value
+
+    def microbench_read(self, pattern):
+        """-> bytes per second of a pure read of V in the access pattern of a sweep kernel (0 linear, 1 rows, 2 x-rows, 3 turn tiles)."""
+        bps = C.c_double(0)
+        self._check(self._L.nhp_microbench_read(self._h, int(pattern), C.byref(bps)), "microbench_read")
+        return bps.value
 
     def launch_count(self):
         return int(self._L.nhp_launch_count(self._h))
