@@ -272,41 +272,21 @@ __global__ void __launch_bounds__(32 * XL_WARPS_V, XL_MINB_V) straight_xl_kernel
         __syncwarp();                                  // the stage is free (row stores of the previous tile have read it)
         const uint32_t tw_cur = tw;
         const int T_cur = T, rows = (tw >> 8) & 63;
-        // Warp-uniform short cut, taken before the tile is even staged: nothing finite travels into the tile on any line and
-        // none of the rows just loaded holds a finite value (they cover the tile and a few vertices of the neighbouring bands,
-        // so the test is only conservative): the relaxation cannot change anything and t stays infinite.
-        bool idle = false;
-        if (!fixed) {
-            uint32_t m0 = 0xffffffffu, m1 = m0, m2 = m0, m3 = m0;
-#pragma unroll
-            for (int r = 0; r < 32; r += 4) {
-                m0 = __viaddmin_u32(nx[r], 0xffffffffu, m0);
-                m1 = __viaddmin_u32(nx[r + 1], 0xffffffffu, m1);
-                m2 = __viaddmin_u32(nx[r + 2], 0xffffffffu, m2);
-                m3 = __viaddmin_u32(nx[r + 3], 0xffffffffu, m3);
-            }
-#pragma unroll
-            for (int r = 32; r < XL_ROWS; r++)
-                if (r < rows) m0 = __viaddmin_u32(nx[r], 0xffffffffu, m0);
-            const uint32_t lowest = min(min(m0, m1), min(m2, m3));
-            idle = __all_sync(0xffffffffu, tv >= VI_INF && lowest >= VI_INF - 1u);
-        }
-        if (!idle) {
+        {
 #pragma unroll
             for (int r = 0; r < XL_ROWS; r++)
                 if (r < 32 || r < rows) stage[r * XL_PITCH + lane] = nx[r];
             stage[XL_DATA + 1 + lane] = (uint32_t)(((tw & 7) * XL_PITCH + lane) * 4);
         }
         const uint4 s0 = ns0, s1 = ns1;
-        __syncwarp();
-        if (s + 1 < NT) {                              // the next tile into the registers the stage has just been filled from
-            T = up ? s + 1 : NT - 2 - s;
+        if (s + 1 < NT) {                              // the next tile into the registers the stage has just been filled from (no
+            T = up ? s + 1 : NT - 2 - s;               // barrier in between: the loads go out as soon as the stores have read them)
             tw = tw_next;
             xl_tile_load<LOG2N>(nx, Vt, tw, T, X0, lane, log2_n);
             if (SOFT) { ns0 = ld_nc16(Sl + 32 * T); ns1 = ld_nc16(Sl + 32 * T + 16); }
             if (s + 2 < NT) tw_next = tab[(up ? s + 2 : NT - 3 - s) * 32];
         }
-        if (idle) continue;
+        __syncwarp();
         uint32_t cm = 0;
         if (up) {
             xl_half<true, SOFT, 0>(row, offs4, tv, wp, w, ct, s0, cm, fixed);
