@@ -8,7 +8,8 @@
 //   S_right[y'][x' / 32][Theta / 4][x' % 32][Theta % 4] = S[Theta][(y' + beta1(Theta)) & M][(x' + beta2(Theta)) & M]     right-turn curves, eq (18)
 //       (tile-major: the four bytes of four consecutive planes of one curve are one word, the 32 curves of a turn tile lie next to
 //       each other, so a warp of the tile kernel reads one 128-byte line per four planes)
-//   S_line [Theta][x'][y'] = S at the vertex eq (23) gives for (x', y', Theta)                straight lines
+//   S_line [Theta][x' / 32][y' / 32][(y' / 16) % 2][x' % 32][y' % 16] = S at the vertex eq (23) gives for (x', y', Theta)     straight lines
+//       (the 16 bytes a thread reads at once next to those of the 31 other lines of its warp)
 // Same bytes, same traffic per pose-update (1 B), three more volumes of N_R bytes in the caller's workspace.
 #include "nhp_internal.cuh"
 
@@ -34,32 +35,35 @@ __global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restri
     }
 }
 
-// One block = a 32 x 32 tile (x', y') of one Theta slice.
+// One block = a 32 x 32 tile (x', y') of one Theta slice: the bytes of 32 neighbouring lines x' = 32 band + l at the steps
+// y' = 32 T + 16 h + e go to S_line[Theta][band][T][h][l][e] -- the 16 bytes (e) a thread of the straight kernels reads at once next to
+// those of the other 31 lines of its warp, so a warp's two loads per tile are 512 contiguous bytes each.
 __global__ void __launch_bounds__(256) soft_line_layout_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
                                                               const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ, int log2_n)
 {
-    __shared__ uint8_t tile[32][33];
+    __shared__ __align__(16) uint8_t tile[32][48];              // [line][step], 16-byte aligned rows
     const int n = 1 << log2_n, mx = n - 1;
     const int t = blockIdx.z, x0 = blockIdx.x << 5, y0 = blockIdx.y << 5;
     const int lane = threadIdx.x, ty = threadIdx.y;
     const int16_t *Bt = B + (size_t)t * n;
     const uint8_t *St = S + ((size_t)t << (2 * log2_n));
-    uint8_t *Ot = Sout + ((size_t)t << (2 * log2_n));
     if ((IJ[t] & 1) == 0) {
-        // eq (23), I = 0: (i, j) = (y', (x' + B(y')) & M): lane = y' is the memory-fast axis of both arrays
+        // eq (23), I = 0: (i, j) = (y', (x' + B(y')) & M): lane = y' is the memory-fast axis
         const int y = y0 + lane, b = Bt[y];
-        for (int r = ty; r < 32; r += 8) {
-            const int x = x0 + r;
-            Ot[((size_t)x << log2_n) + y] = St[((size_t)((x + b) & mx) << log2_n) + y];
-        }
+        for (int r = ty; r < 32; r += 8) tile[r][lane] = St[((size_t)((x0 + r + b) & mx) << log2_n) + y];
     } else {
-        // I = 1: (i, j) = ((x' + B(y')) & M, y'): read with lane = x', write with lane = y'
+        // I = 1: (i, j) = ((x' + B(y')) & M, y'): lane = x' is the memory-fast axis
         for (int r = ty; r < 32; r += 8) {
             const int y = y0 + r;
-            tile[r][lane] = St[((size_t)y << log2_n) + ((x0 + lane + Bt[y]) & mx)];
+            tile[lane][r] = St[((size_t)y << log2_n) + ((x0 + lane + Bt[y]) & mx)];
         }
-        __syncthreads();
-        for (int r = ty; r < 32; r += 8) Ot[((size_t)(x0 + r) << log2_n) + y0 + lane] = tile[lane][r];
+    }
+    __syncthreads();
+    const int k = ty * 32 + lane;                               // 64 threads write one 16-byte piece each: k = 32 h + l
+    if (k < 64) {
+        const int h = k >> 5, l = k & 31;
+        uint4 *out = (uint4 *)(Sout + ((size_t)t << (2 * log2_n)) + (((size_t)blockIdx.x << (log2_n - 5)) + blockIdx.y) * 1024);
+        out[k] = *(const uint4 *)&tile[l][16 * h];
     }
 }
 

@@ -253,8 +253,8 @@ __global__ void __launch_bounds__(32 * XL_WARPS_V, XL_MINB_V) straight_xl_kernel
     const int NT = 1 << (log2_n - 5);
     unsigned long long Vt = (unsigned long long)(V + ((size_t)t << (2 * log2_n)));
     asm volatile("" : "+l"(Vt));
-    // S_line[Theta][x'][y']: this thread's line, 32 bytes per tile
-    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) + ((size_t)(X0 + lane) << log2_n) : nullptr;
+    // S_line[Theta][band][T][half][lane][16] (softlayout.cu): this thread's line, two 16-byte pieces per tile, 1024 bytes from tile to tile
+    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) + (((size_t)(X0 >> 5) << (log2_n - 5)) << 10) + 16 * lane : nullptr;
     uint32_t *stage = smem + warp * XL_STAGE;
     char *row = (char *)(stage + lane * XL_PITCH);
     const uint4 *offs4 = (const uint4 *)(stage + XL_DATA + 1);                  // 16-byte aligned: XL_DATA + 1 = 1288
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(32 * XL_WARPS_V, XL_MINB_V) straight_xl_kernel
     int T = up ? 0 : NT - 1;
     uint32_t tw = tab[T * 32], tw_next = NT > 1 ? tab[(up ? 1 : NT - 2) * 32] : 0u;
     xl_tile_load<LOG2N>(nx, Vt, tw, T, X0, lane, log2_n);
-    if (SOFT) { ns0 = ld_nc16(Sl + 32 * T); ns1 = ld_nc16(Sl + 32 * T + 16); }
+    if (SOFT) { ns0 = ld_nc16(Sl + 1024 * T); ns1 = ld_nc16(Sl + 1024 * T + 512); }
     uint32_t tv = VI_INF, wp = SOFT ? 0u : w;          // nothing arrives at the wall cell the line starts from
 #pragma unroll 1
     for (int s = 0; s < NT; s++) {
@@ -283,7 +283,7 @@ __global__ void __launch_bounds__(32 * XL_WARPS_V, XL_MINB_V) straight_xl_kernel
             T = up ? s + 1 : NT - 2 - s;               // barrier in between: the loads go out as soon as the stores have read them)
             tw = tw_next;
             xl_tile_load<LOG2N>(nx, Vt, tw, T, X0, lane, log2_n);
-            if (SOFT) { ns0 = ld_nc16(Sl + 32 * T); ns1 = ld_nc16(Sl + 32 * T + 16); }
+            if (SOFT) { ns0 = ld_nc16(Sl + 1024 * T); ns1 = ld_nc16(Sl + 1024 * T + 512); }
             if (s + 2 < NT) tw_next = tab[(up ? s + 2 : NT - 3 - s) * 32];
         }
         __syncwarp();
@@ -326,7 +326,7 @@ __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restr
     const int16_t *Bt = B + (size_t)t * n;
     unsigned long long Vt = (unsigned long long)(V + ((size_t)t << (2 * log2_n)));
     asm volatile("" : "+l"(Vt));
-    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) + ((size_t)(X0 + lane) << log2_n) : nullptr;
+    const uint8_t *Sl = SOFT ? Sline + ((size_t)t << (2 * log2_n)) + (((size_t)(X0 >> 5) << (log2_n - 5)) << 10) + 16 * lane : nullptr;
     const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
     const uint32_t c0 = (uint32_t)(X0 + lane);
     const int NT = n >> 5;
@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restr
             u[k] = *(const uint32_t *)(Vt + 4ull * off);
         }
         uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
-        if (SOFT) { s0 = ld_nc16(Sl + 32 * T); s1 = ld_nc16(Sl + 32 * T + 16); }
+        if (SOFT) { s0 = ld_nc16(Sl + 1024 * T); s1 = ld_nc16(Sl + 1024 * T + 512); }
         uint32_t cm = 0;
         if (!fixed && tile_is_idle4(u, tv)) { }
         else if (up) RelaxLoop<true, SOFT>::run(u, tv, wp, w, ct, s0, s1, cm);
@@ -419,8 +419,8 @@ __global__ void __launch_bounds__(512) straight_sect_kernel(uint32_t *__restrict
     const uint32_t w = SOFT ? lenq[t] << 4 : lenq[t];
     uint4 s0 = make_uint4(0, 0, 0, 0), s1 = s0;
     if (SOFT) {
-        const uint8_t *Sl = Sline + ((size_t)t << (2 * log2_n)) + ((size_t)(X0 + lane) << log2_n) + 32 * T;
-        s0 = ld_nc16(Sl); s1 = ld_nc16(Sl + 16);
+        const uint8_t *Sl = Sline + ((size_t)t << (2 * log2_n)) + ((((size_t)blockIdx.x << (log2_n - 5)) + T) << 10) + 16 * lane;
+        s0 = ld_nc16(Sl); s1 = ld_nc16(Sl + 512);
     }
     uint32_t u[32];
     uint32_t tw = 0;
