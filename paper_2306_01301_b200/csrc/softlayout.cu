@@ -13,25 +13,25 @@
 // Same bytes, same traffic per pose-update (1 B), three more volumes of N_R bytes in the caller's workspace.
 #include "nhp_internal.cuh"
 
-// One block = 32 neighbouring curves (x' = x0 .. x0 + 31 at one y') of one turn family: gather their N_theta planes
-// (32-byte row segments) into shared memory, write each curve's N_theta bytes out contiguously.
+// One block = 32 neighbouring curves (x' = x0 .. x0 + 31 at one y') of one turn family, lane = curve.  A warp produces the words
+// j = warp, warp + nwarps, ...: four byte loads (the curve's vertices in the planes 4 j .. 4 j + 3, each a 32-byte row segment for
+// the warp) packed into one word, stored as one 128-byte line -- no shared memory, no barrier.
 __global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
                                                               const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
 {
-    extern __shared__ __align__(16) uint8_t tile[];             // [32][nt + 4]: an odd number of words per curve
-    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2, stride = nt + 4;
+    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int x0 = blockIdx.x << 5, yp = blockIdx.y;
-    for (int t = warp; t < nt; t += nwarps) {
-        const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];
-        tile[lane * stride + t] = S[((((size_t)t << log2_n) + ((yp + bb) & mx)) << log2_n) + ((x0 + ba + lane) & mx)];
-    }
-    __syncthreads();
-    // tile-major: word j = planes 4 j .. 4 j + 3 of a curve, the 32 curves of the tile next to each other (one 128-byte line)
     uint32_t *out = (uint32_t *)Sout + (((size_t)yp << (log2_n - 5)) + blockIdx.x) * ((size_t)nt * 8);
-    for (int c = threadIdx.x; c < 8 * nt; c += blockDim.x) {
-        const int j = c >> 5, curve = c & 31;
-        out[c] = *(const uint32_t *)(tile + curve * stride + 4 * j);
+    for (int j = warp; j < (nt >> 2); j += nwarps) {
+        uint32_t word = 0;
+#pragma unroll
+        for (int e = 0; e < 4; e++) {
+            const int t = 4 * j + e;
+            const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];
+            word |= (uint32_t)S[((((size_t)t << log2_n) + ((yp + bb) & mx)) << log2_n) + ((x0 + ba + lane) & mx)] << (8 * e);
+        }
+        out[j * 32 + lane] = word;
     }
 }
 
@@ -70,9 +70,8 @@ __global__ void __launch_bounds__(256) soft_line_layout_kernel(uint8_t *__restri
 int launch_soft_layouts(nhp_planner *p)
 {
     const int n = p->n, nt = p->nt;
-    const size_t smem = (size_t)32 * (nt + 4);
-    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
-    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, smem, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
+    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
+    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
     soft_line_layout_kernel<<<dim3(n / 32, n / 32, nt), dim3(32, 8), 0, p->stream>>>(p->S_line, p->S, p->d_B, p->d_IJ, p->log2_n);
     return 3;
 }
@@ -80,5 +79,5 @@ int launch_soft_layouts(nhp_planner *p)
 // function attributes are per device: set for the handle's device at creation (nhp_planner_create)
 int set_softlayout_attributes()
 {
-    return cudaFuncSetAttribute(soft_turn_layout_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * (4096 + 16)) == cudaSuccess ? NHP_OK : NHP_E_CUDA;
+    return NHP_OK;                 // (no kernel of this file needs more than the default shared memory any more)
 }
