@@ -118,30 +118,34 @@ __global__ void __launch_bounds__(192) backtrack_kernel(const uint32_t *__restri
                     const uint32_t u = uu[c];
                     const unsigned blk = __ballot_sync(0xffffffffu, u == 0u);       // blocked (or past the end)
                     const int first = blk ? __ffs(blk) - 1 : 32;
-                    unsigned long long pre = (lane < first) ? ww[c] : 0;             // inclusive prefix sum of w
+                    // inclusive prefix sum of the 32 edge weights of the chunk (each < 2^26: no wrap in 32 bits), then the running total
+                    uint32_t p32 = (lane < first) ? ww[c] : 0u;
 #pragma unroll
                     for (int d = 1; d < 32; d <<= 1) {
-                        const unsigned long long y = __shfl_up_sync(0xffffffffu, pre, d);
-                        if (lane >= d) pre += y;
+                        const uint32_t y = __shfl_up_sync(0xffffffffu, p32, d);
+                        if (lane >= d) p32 += y;
                     }
-                    pre += E;
-                    unsigned long long key = KINF;
-                    uint32_t seg = 0;
+                    const unsigned long long pre = E + p32;
                     if (lane < first && u < VI_INF) {
                         // u == 1 (cost 0) only at the start vertex: the maneuver in progress there is entered for free
                         const uint32_t ctm = (m == P.m0 && u == 1u && at_start[c]) ? 0u : ct;
                         const unsigned long long cand = (unsigned long long)(u - 1u) + ctm + pre;
-                        if (cand < NHP_COST_LIMIT) { key = (cand << 13) | (unsigned)k; seg = (uint32_t)(ctm + pre); }
+                        if (cand < NHP_COST_LIMIT) {
+                            // every lane keeps its own best; (cost, steps back) is the key, so the warp-wide minimum taken once at the
+                            // end is the nearest source of least cost (DESIGN R19) whatever chunk it came from
+                            const unsigned long long key = (cand << 13) | (unsigned)k;
+                            if (key < best) { best = key; best_seg = (uint32_t)(ctm + pre); }
+                        }
                     }
-                    const unsigned long long kmin = warp_min_u64(key);
-                    if (kmin < best) {                               // strictly smaller: earlier chunks win ties
-                        best = kmin;
-                        const unsigned who = __ballot_sync(0xffffffffu, key == kmin);
-                        best_seg = __shfl_sync(0xffffffffu, seg, __ffs(who) - 1);
-                    }
-                    E = __shfl_sync(0xffffffffu, pre, 31);
+                    E += __shfl_sync(0xffffffffu, p32, 31);
                     if (first < 32) done = true;
                 }
+            }
+            {
+                const unsigned long long kmin = warp_min_u64(best);
+                const unsigned who = __ballot_sync(0xffffffffu, best == kmin);
+                best_seg = __shfl_sync(0xffffffffu, best_seg, __ffs(who) - 1);
+                best = kmin;
             }
             if (best != KINF) cell((int)(best & 0x1fffu), bi, bj, bt);
         }
