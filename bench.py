@@ -126,6 +126,16 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def bench_config(sc, n_cycles, args, ws, dt_dev=False):
+    """The `config` object of the JSON line: the workload and how it is run, the same keys for both arms."""
+    n_r = sc.n * sc.n * sc.nt
+    return {"workload": workload_name(sc, n_cycles), "baseline_config": args.config, "pose_updates_per_plan": 6 * n_cycles * n_r,
+            "parallelism": f"replicas x{ws} (no collective)",
+            "soft_image": ("device distance transform" if dt_dev else "harness (CPU)") if sc.soft is not None else None,
+            "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
+            "fixed_work": bool(args.fixed_work), "no_shortcuts": bool(args.no_shortcuts)}
+
+
 def pick_goal(p, sc, torch):
     """The nominal goal if the sweeps reached it, else the reached candidate of largest finite cost
     (N_T cycles only guarantee plans of <= N_T maneuvers).  Harness logic on <= 257 values."""
@@ -358,11 +368,8 @@ def run_ours(args):
         "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config,
-                   "pose_updates_per_plan": updates_per_plan, "parallelism": f"replicas x{ws} (no collective)", "soft_image": ("device distance transform" if dt_dev else "harness (CPU)") if sc.soft is not None else None,
-                   "l2": f"inputs larger than L2: value volume {4 * n_r / 2**20:.0f} MiB vs 126 MB L2, every sweep streams it",
-                   "fixed_work": bool(args.fixed_work), "no_shortcuts": bool(args.no_shortcuts),
-                   "goal": list(b.goal), "plan_waypoints": len(plan), "plan_cost": cost},
+        "config": bench_config(sc, n_cycles, args, ws, dt_dev),
+        "result": {"goal": list(b.goal), "plan_waypoints": len(plan), "plan_cost": cost},
         "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
         "clocks": clk,
         "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
@@ -511,7 +518,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": ws, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "u32", "data": "synthetic",
-        "config": {"workload": workload_name(sc, n_cycles), "baseline_config": args.config},
+        "config": bench_config(sc, n_cycles, args, ws),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": int(o.threads), "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
