@@ -565,20 +565,31 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     unsigned long long before = 0, after = 0;
     // `fixed` (NHP_FLAG_FIXED_WORK / NHP_FLAG_NO_SHORTCUTS) switches the three short cuts off; fixed == 1 also stores every row: the same
     // instructions and bytes whatever the volume holds
-    uint32_t top = col[0];
+    // Short-cut conditions (warp-uniform).  Hard costs: the minimum over (v - 1) with wrap-around (blocked 0 -> 2^32 - 1, unreached
+    // -> 2^30, finite below) tells both "every vertex of the warp is blocked" and "no finite value in this warp yet"; four
+    // independent chains.  Soft costs (no no_finite short cut): a max tree for "all blocked".
+    bool all_blocked = false, no_finite = false;
+    if (!fixed) {
+        if (SOFT) {
+            uint32_t top = col[0];
 #pragma unroll
-    for (int k = 1; k + 1 < L; k += 2) top = __vimax3_u32(top, col[k], col[k + 1]);
-    const bool all_blocked = !fixed && __all_sync(0xffffffffu, max(top, col[L - 1]) == 0u);
-    // (soft kernels keep one chain variant: a second copy of their loops costs registers they do not have)
-    const bool none_blocked = !SOFT && !fixed && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
-    // "no finite value in this warp yet": min over (v - 1) with wrap-around (blocked 0 -> 2^32 - 1, unreached -> 2^30)
-    bool no_finite = false;
-    if (!SOFT && !fixed) {
-        uint32_t lowest = 0xffffffffu;
+            for (int k = 1; k + 1 < L; k += 2) top = __vimax3_u32(top, col[k], col[k + 1]);
+            all_blocked = __all_sync(0xffffffffu, max(top, col[L - 1]) == 0u);
+        } else {
+            uint32_t m0 = 0xffffffffu, m1 = m0, m2 = m0, m3 = m0;
 #pragma unroll
-        for (int k = 0; k < L; k++) lowest = __viaddmin_u32(col[k], 0xffffffffu, lowest);
-        no_finite = __all_sync(0xffffffffu, lowest >= VI_INF - 1u);
+            for (int k = 0; k < L; k += 4) {
+                m0 = __viaddmin_u32(col[k], 0xffffffffu, m0);
+                m1 = __viaddmin_u32(col[k + 1], 0xffffffffu, m1);
+                m2 = __viaddmin_u32(col[k + 2], 0xffffffffu, m2);
+                m3 = __viaddmin_u32(col[k + 3], 0xffffffffu, m3);
+            }
+            const uint32_t lowest = min(min(m0, m1), min(m2, m3));
+            all_blocked = __all_sync(0xffffffffu, lowest == 0xffffffffu);
+            no_finite = __all_sync(0xffffffffu, lowest >= VI_INF - 1u);
+        }
     }
+    const bool none_blocked = !SOFT && !fixed && __all_sync(0xffffffffu, !blocked_lo && !blocked_hi);
     bool ran_a, ran_last, tile_idle = false;
     if constexpr (SOFT) {
         const bool blocked_any = blocked_lo || blocked_hi;
