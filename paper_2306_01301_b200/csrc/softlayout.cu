@@ -35,6 +35,36 @@ __global__ void __launch_bounds__(256) soft_turn_layout_kernel(uint8_t *__restri
     }
 }
 
+// The same for grids of at least 128 cells per side, four tiles (128 neighbouring curves) per block and four curves per lane: per
+// plane two aligned 4-byte loads (wrapped on the torus per lane) and a funnel shift give the lane's four bytes whatever the
+// alignment of the row segment; the 4 x 4 bytes of four planes are transposed in registers (eight PRMT) into the four output
+// words, stored as one 16-byte piece.  Four times fewer load instructions per byte than soft_turn_layout_kernel.
+__global__ void __launch_bounds__(256) soft_turn_layout4_kernel(uint8_t *__restrict__ Sout, const uint8_t *__restrict__ S,
+                                                               const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb)
+{
+    const int mx = (1 << log2_n) - 1, mt = nt - 1, quarter = nt >> 2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int x0 = blockIdx.x << 7, yp = blockIdx.y;
+    // tile (yp, 4 blockIdx.x + lane / 8), word j, curves 4 (lane % 8) .. + 3
+    uint32_t *out = (uint32_t *)Sout + (((size_t)yp << (log2_n - 5)) + 4 * blockIdx.x + (lane >> 3)) * ((size_t)nt * 8) + 4 * (lane & 7);
+    for (int j = warp; j < (nt >> 2); j += nwarps) {
+        uint32_t W[4];
+#pragma unroll
+        for (int e = 0; e < 4; e++) {
+            const int t = 4 * j + e;
+            const int ba = beta[(t + qa * quarter) & mt], bb = beta[(t + qb * quarter) & mt];
+            const uint8_t *row = S + ((((size_t)t << log2_n) + ((yp + bb) & mx)) << log2_n);
+            const int c = (x0 + ba + 4 * lane) & mx, c0 = c & ~3;           // (c & 3 is the same in every lane: N is a multiple of 4)
+            const uint32_t w0 = *(const uint32_t *)(row + c0), w1 = *(const uint32_t *)(row + ((c0 + 4) & mx));
+            W[e] = __funnelshift_r(w0, w1, 8 * (c & 3));
+        }
+        const uint32_t t0 = __byte_perm(W[0], W[1], 0x5140), t1 = __byte_perm(W[2], W[3], 0x5140);
+        const uint32_t t2 = __byte_perm(W[0], W[1], 0x7362), t3 = __byte_perm(W[2], W[3], 0x7362);
+        *(uint4 *)(out + j * 32) = make_uint4(__byte_perm(t0, t1, 0x5410), __byte_perm(t0, t1, 0x7632), __byte_perm(t2, t3, 0x5410),
+                                              __byte_perm(t2, t3, 0x7632));
+    }
+}
+
 // One block = a 32 x 32 tile (x', y') of one Theta slice: the bytes of 32 neighbouring lines x' = 32 band + l at the steps
 // y' = 32 T + 16 h + e go to S_line[Theta][band][T][h][l][e] -- the 16 bytes (e) a thread of the straight kernels reads at once next to
 // those of the other 31 lines of its warp, so a warp's two loads per tile are 512 contiguous bytes each.
@@ -70,8 +100,13 @@ __global__ void __launch_bounds__(256) soft_line_layout_kernel(uint8_t *__restri
 int launch_soft_layouts(nhp_planner *p)
 {
     const int n = p->n, nt = p->nt;
-    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
-    soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
+    if (n >= 128) {
+        soft_turn_layout4_kernel<<<dim3(n / 128, n), 256, 0, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
+        soft_turn_layout4_kernel<<<dim3(n / 128, n), 256, 0, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
+    } else {
+        soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_left, p->S, p->d_beta, p->log2_n, nt, 0, 3);
+        soft_turn_layout_kernel<<<dim3(n / 32, n), 256, 0, p->stream>>>(p->S_right, p->S, p->d_beta, p->log2_n, nt, 2, 1);
+    }
     soft_line_layout_kernel<<<dim3(n / 32, n / 32, nt), dim3(32, 8), 0, p->stream>>>(p->S_line, p->S, p->d_B, p->d_IJ, p->log2_n);
     return 3;
 }
