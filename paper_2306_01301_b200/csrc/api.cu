@@ -426,7 +426,7 @@ int nhp_run_nturn_from(nhp_planner *p, int i, int j, int theta, int m0, int n_cy
     p->launches += launch_init_volume(p, i, j, theta);
     p->canonical = false;
     if (m0 >= 0) p->launches += launch_seed_in_progress(p, m0);
-    p->launches += launch_cycles(p, n_cycles);
+    p->launches += launch_cycles(p, n_cycles, true);
     CU(cudaGetLastError());
     p->have_run = true;
     return NHP_OK;
@@ -499,7 +499,7 @@ int nhp_run_more(nhp_planner *p, int n_cycles)
     if (n_cycles <= 0) return fail(p, NHP_E_ARG, "n_cycles must be positive");
     DeviceGuard guard(p);
     if (p->canonical) { p->launches += launch_export_volume(p, false); p->canonical = false; }
-    p->launches += launch_cycles(p, n_cycles);
+    p->launches += launch_cycles(p, n_cycles, false);
     CU(cudaGetLastError());
     return NHP_OK;
 }

@@ -190,7 +190,7 @@ int finish_footprint(nhp_planner *p);                 // host: run lists into th
 int launch_render(nhp_planner *p, bool soft);
 int launch_init_volume(nhp_planner *p, int si, int sj, int st);
 int launch_export_volume(nhp_planner *p, bool to_canonical);
-int launch_cycles(nhp_planner *p, int n_cycles);
+int launch_cycles(nhp_planner *p, int n_cycles, bool fresh);   // fresh: the volume has just been initialised (one finite vertex)
 int build_cycle_graph(nhp_planner *p);               // at creation; NHP_OK also when no graph is built
 int launch_backtrack(nhp_planner *p, int gi, int gj, int gt);     // gi < 0: the goal comes from launch_goal_search
 int launch_goal_search(nhp_planner *p, int n_goals, int d, uint32_t W, uint32_t w);

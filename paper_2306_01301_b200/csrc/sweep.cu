@@ -521,14 +521,15 @@ __device__ __forceinline__ void tile_rows_store(const uint32_t (&col)[L], uint32
 template <int L, int NPASS, bool UP0, bool SOFT>
 __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Scurve,
                                                           const int16_t *__restrict__ beta, int log2_n, int nt, int qa, int qb,
-                                                          TurnPass pa, TurnPass pb, uint32_t one, int fixed)
+                                                          TurnPass pa, TurnPass pb, uint32_t one, int fixed, int bx0, int by0)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int S = nt / L, mt = nt - 1, quarter = nt >> 2, mx = (1 << log2_n) - 1;
     uint32_t *so = smem;                                      // [nt] element index of the tile's first vertex in every plane
     uint2 *sMD = (uint2 *)(so + nt);                          // [2][2 S][32] (M, D) of every section (twice), one set per maneuver
     const int lane = threadIdx.x & 31, sec = threadIdx.x >> 5;
-    const int x0 = blockIdx.x << 5, yp = blockIdx.y;
+    const int bx = blockIdx.x + bx0;                          // (bx0, by0): first tile of the launch; (0, 0) and a full grid but for the
+    const int x0 = bx << 5, yp = blockIdx.y + by0;            // very first LF of a plan, see launch_cycles
     // every warp fills in the rows of its own 32 planes: no CTA-wide barrier stands between the start of a tile and its loads
     int seam;
     {
@@ -544,7 +545,7 @@ __global__ void __launch_bounds__(1024, 1) turn_tile_kernel(uint32_t *__restrict
     // tile-major soft volume (softlayout.cu): tile (yp, x0 / 32) = nt / 4 lines of 32 words; this section's words 8 sec .. 8 sec + 7
     const uint32_t *sp = nullptr;
     if (SOFT) {
-        sp = (const uint32_t *)Scurve + (((size_t)yp << (log2_n - 5)) + blockIdx.x) * ((size_t)nt * 8) + (size_t)sec * (L / 4) * 32;
+        sp = (const uint32_t *)Scurve + (((size_t)yp << (log2_n - 5)) + bx) * ((size_t)nt * 8) + (size_t)sec * (L / 4) * 32;
         if (lane < L / 4) asm volatile("prefetch.global.L1 [%0];" ::"l"(sp + lane * 32));       // the section's eight lines, needed after the tile
         sp += lane;
     }
@@ -631,7 +632,7 @@ static int turn_tile_L(const nhp_planner *p)
 }
 
 // One launch = maneuver ma (and then mb, the opposite direction on the same curve family, if mb >= 0).
-static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
+static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb, int only_bx = -1, int only_by = -1)
 {
     const int n = p->n, nt = p->nt, S = nt / L;
     const bool soft = p->S != nullptr;
@@ -647,10 +648,12 @@ static int launch_turn_tile(nhp_planner *p, int L, int ma, int mb)
     const TurnPass pa = pass(ma), pb = pass(mb);
     const uint8_t *Sc = left ? p->S_left : p->S_right;
     const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : (p->w.flags & NHP_FLAG_NO_SHORTCUTS) ? 2 : 0;   // 1: no short cuts, store all; 2: no short cuts
-    const dim3 grid(n / 32, n), block(32 * S);
+    const bool one_tile = only_bx >= 0;
+    const dim3 grid(one_tile ? 1 : n / 32, one_tile ? 1 : n), block(32 * S);
+    const int bx0 = one_tile ? only_bx : 0, by0 = one_tile ? only_by : 0;
     const size_t smem = sizeof(uint32_t) * (size_t)nt + sizeof(uint2) * 4 * (size_t)S * 32;
     ProfScope prof(p, mb >= 0 ? 11 : ma);
-#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u, fixed)
+#define NHP_TT(NP, UP, SO) turn_tile_kernel<32, NP, UP, SO><<<grid, block, smem, p->stream>>>(p->V, Sc, p->d_beta, p->log2_n, nt, qa, qb, pa, pb, 1u, fixed, bx0, by0)
 #define NHP_TT2(NP, UP) do { if (soft) NHP_TT(NP, UP, true); else NHP_TT(NP, UP, false); } while (0)
     if (mb >= 0) { if (up) NHP_TT2(2, true); else NHP_TT2(2, false); }
     else { if (up) NHP_TT2(1, true); else NHP_TT2(1, false); }
@@ -713,7 +716,7 @@ int build_cycle_graph(nhp_planner *p)
 // Cycle driver, PAPER.md:392 + l.475: LF, SF, RB, RF, SB, LB per cycle.  FORWARD_ONLY keeps LF, SF, RF.
 // With the tile kernel, RB+RF run as one launch and LB is fused with the LF of the NEXT cycle (same curve family,
 // adjacent in the sequence), so the order of operations on every vertex is exactly the paper's.
-int launch_cycles(nhp_planner *p, int n_cycles)
+int launch_cycles(nhp_planner *p, int n_cycles, bool fresh)
 {
     int launches = 0;
     const bool fwd_only = p->w.flags & NHP_FLAG_FORWARD_ONLY;
@@ -732,7 +735,16 @@ int launch_cycles(nhp_planner *p, int n_cycles)
         } else if (fwd_only) {
             launches += inner();
         } else {
-            if (c == 0) launches += launch_turn_tile(p, L, M_LF, -1);
+            if (c == 0) {
+                // The very first LF of a plan finds one finite vertex, the start: only the left-turn curve through it can change
+                // (PAPER.md:392 step 5; eq (18) inverted gives its thread coordinates), so one tile is launched instead of N^2 / 32.
+                // Not with a maneuver in progress at the start (more seeds) and not in the fixed-work modes.
+                if (fresh && p->start_m0 < 0 && !(p->w.flags & (NHP_FLAG_FIXED_WORK | NHP_FLAG_NO_SHORTCUTS))) {
+                    const int mt = p->nt - 1, mx = p->n - 1, q = p->nt >> 2, th = p->start[2];
+                    const int xp = (p->start[0] - p->beta[th & mt]) & mx, yp = (p->start[1] - p->beta[(th + 3 * q) & mt]) & mx;
+                    launches += launch_turn_tile(p, L, M_LF, -1, xp >> 5, yp);
+                } else launches += launch_turn_tile(p, L, M_LF, -1);
+            }
             if (c + 1 < n_cycles) launches += inner();
             else {
                 launches += launch_straight(p, M_SF);
