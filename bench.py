@@ -245,6 +245,8 @@ class PlanBench:
             ms, n = kt.get(k, (0.0, 0))
             if not n:
                 continue
+            if k == "LF" and not (self.p.flags & (self.nhp.FLAG_FIXED_WORK | self.nhp.FLAG_NO_SHORTCUTS)):
+                continue            # the first LF of a plan is one tile (the curve through the start), not a sweep of the volume
             avg = ms / n
             alg = alg_b * self.updates_per_launch(k)
             tr = measured_traffic(config, k)
