@@ -502,6 +502,8 @@ def test_straight_sections_and_streaming_at_the_other_sizes(mods):
     _sweeps_match(mods, scenes.get_config(4), nhp.FLAG_SECTIONS, 2)                                          # ... with soft costs
     _sweeps_match(mods, scenes.get_config(3), nhp.FLAG_SECTIONS | nhp.FLAG_FIXED_WORK, 1)
     _sweeps_match(mods, scenes.random_scene(11, 6, 8, 22, vehicle=(9, 4), n_rects=60, n_cycles=1), 0, 1)     # N = 2048: streaming
+    _sweeps_match(mods, scenes.random_scene(5, 11, 6, 23, n_cycles=1), 0, 2)                                 # N_theta = 2048: turn sweeps
+                                                                                                             # by the thread-per-curve kernels
 
 
 def test_no_write_outside_the_buffers_and_run_to_run_identical(mods):
