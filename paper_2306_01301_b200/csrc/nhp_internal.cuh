@@ -117,6 +117,7 @@ struct nhp_planner {
     // nhp_reach_run), number of levels of the last run, its start
     uint32_t *r_levels = nullptr, *r_Lt = nullptr, *r_Ct = nullptr, *r_Gt = nullptr;   // in the caller's workspace
     int r_n_levels = -1, r_start[3] = {0, 0, 0};
+    int sparse_xp = -1, sparse_yp = -1;   // >= 0 only while launch_cycles launches the first SF of a plan (straight.cu: StartCurve)
     int start_m0 = -1;             // maneuver in progress at the start (nhp_run_nturn_from), -1 = none
     // plan extraction
     int32_t *d_status = nullptr;   // N-turn planner: [0] start blocked, [1] backtrack rc, [2] count, [3] cost, [4..7] goal search:

@@ -29,6 +29,22 @@ __device__ __forceinline__ uint4 ld_nc16(const uint8_t *p)
     return q;
 }
 
+// The first SF of a plan (launch_cycles): the only finite vertices are those of the left-turn curve through the start, one per
+// Theta plane, so in every slice only the line through that vertex can change and only its band is launched.  xp < 0: off.
+struct StartCurve {
+    int xp, yp, nt;                  // thread coordinates of the curve, eq (18) inverted at the start
+    const int16_t *beta, *B;
+};
+
+// line x' of slice t (I = 0 or 1, eq (23) inverted) through the start curve's vertex in plane t
+template <int I>
+__device__ __forceinline__ int start_curve_line(const StartCurve &sc, int t, int log2_n)
+{
+    const int n = 1 << log2_n, mx = n - 1, mt = sc.nt - 1, q = sc.nt >> 2;
+    const int i = (sc.xp + sc.beta[t & mt]) & mx, j = (sc.yp + sc.beta[(t + 3 * q) & mt]) & mx;      // eq (18), left family (beta0, beta3)
+    return I ? (i - sc.B[(size_t)t * n + j]) & mx : (j - sc.B[(size_t)t * n + i]) & mx;
+}
+
 // Relax the 32 steps of a tile for this thread's line (Insert 5, internal encoding, in the form
 // of nhp_arrive: the value travels as t = value AT the vertex minus ct, wp = the pending edge weight of the vertex
 // behind it):   t = min(t + wp, u);  V[i] = min(t + ct, u);  t = infinity behind a blocked vertex.
@@ -243,12 +259,12 @@ template <bool SOFT, int LOG2N>
 __global__ void __launch_bounds__(32 * XL_WARPS_V, XL_MINB_V) straight_xl_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
                                                                                const uint32_t *__restrict__ xl_tab, const uint8_t *__restrict__ IJ,
                                                                                const int16_t *__restrict__ tlist, const uint32_t *__restrict__ lenq,
-                                                                               uint32_t ct, int log2_n, int is_forward, int fixed)
+                                                                               uint32_t ct, int log2_n, int is_forward, int fixed, StartCurve sc)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const int xs = blockIdx.y, t = tlist[xs];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
+    const int X0 = sc.xp >= 0 ? (start_curve_line<0>(sc, t, log2_n) & ~31) : (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
     const bool up = (is_forward == ((IJ[t] >> 1) & 1));                         // eq (24)
     const int NT = 1 << (log2_n - 5);
     unsigned long long Vt = (unsigned long long)(V + ((size_t)t << (2 * log2_n)));
@@ -316,11 +332,13 @@ template <bool SOFT>
 __global__ void __launch_bounds__(128, 7) straight_rows_kernel(uint32_t *__restrict__ V, const uint8_t *__restrict__ Sline,
                                                             const int16_t *__restrict__ B, const uint8_t *__restrict__ IJ,
                                                             const int16_t *__restrict__ tlist,
-                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward, int fixed)
+                                                            const uint32_t *__restrict__ lenq, uint32_t ct, int log2_n, int is_forward, int fixed,
+                                                            StartCurve sc)
 {
     const int n = 1 << log2_n, mx = n - 1, t = tlist[blockIdx.y];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int X0 = (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
+    // (sparse first SF: the CTA's four warps take the aligned group of four bands that holds the line)
+    const int X0 = sc.xp >= 0 ? (((start_curve_line<1>(sc, t, log2_n) >> 5) & ~3) + warp) << 5 : (blockIdx.x * (blockDim.x >> 5) + warp) << 5;
     const int jpos = (IJ[t] >> 1) & 1;
     const bool up = (is_forward == jpos);                                       // eq (24)
     const int16_t *Bt = B + (size_t)t * n;
@@ -495,6 +513,8 @@ __global__ void __launch_bounds__(512) straight_sect_kernel(uint32_t *__restrict
 // and one for those with I = 1 (tiles in registers).  Returns the number of kernels launched (0 = not applicable).
 int launch_straight_tile(nhp_planner *p, int m)
 {
+    const bool sparse = p->sparse_xp >= 0;
+    const StartCurve sc{p->sparse_xp, p->sparse_yp, p->nt, p->d_beta, p->d_B};
     if (p->w.flags & NHP_FLAG_SIMPLE_KERNELS) return 0;
     const bool soft = p->S != nullptr;
     const int n = p->n, nt = p->nt;
@@ -502,11 +522,11 @@ int launch_straight_tile(nhp_planner *p, int m)
     ProfScope prof(p, m);
     const uint32_t *lenq = p->d_lenq + (size_t)m * nt;
     const int nx = p->n_xslices, ny = nt - nx;
-    const dim3 gy(bands / warps, ny);
+    const dim3 gy(sparse ? 1 : bands / warps, ny);
     const int fwd = (m == M_SF);
     const int fixed = (p->w.flags & NHP_FLAG_FIXED_WORK) ? 1 : (p->w.flags & NHP_FLAG_NO_SHORTCUTS) ? 2 : 0;   // 1: no short cuts, store all; 2: no short cuts
     // Sections (one warp per tile, all tiles of a band at once): small grids, or on request; at most 16 tiles per line
-    if (bands <= 16 && !(p->w.flags & NHP_FLAG_NO_SECTIONS) && (n <= 256 || (p->w.flags & NHP_FLAG_SECTIONS))) {
+    if (!sparse && bands <= 16 && !(p->w.flags & NHP_FLAG_NO_SECTIONS) && (n <= 256 || (p->w.flags & NHP_FLAG_SECTIONS))) {
         const size_t smx = sizeof(uint32_t) * (size_t)bands * (64 + XL_STAGE);
         ProfScope ps(p, 16);                                     // both slice groups in ONE launch (the block index tells which)
         if (soft) straight_sect_kernel<true><<<dim3(bands, nt), bands * 32, smx, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, p->d_tlist, nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
@@ -517,9 +537,9 @@ int launch_straight_tile(nhp_planner *p, int m)
     {
         const int xw = bands < XL_WARPS_V ? bands : XL_WARPS_V;
         const size_t smem = sizeof(uint32_t) * (size_t)xw * XL_STAGE;
-        const dim3 gx(bands / xw, nx);
+        const dim3 gx(sparse ? 1 : bands / xw, nx);
         ProfScope px(p, 14);
-#define NHP_XL(SO, L2N) straight_xl_kernel<SO, L2N><<<gx, xw * 32, smem, p->stream>>>(p->V, p->S_line, p->d_xl_tab, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed)
+#define NHP_XL(SO, L2N) straight_xl_kernel<SO, L2N><<<gx, xw * 32, smem, p->stream>>>(p->V, p->S_line, p->d_xl_tab, p->d_IJ, p->d_tlist, lenq, p->w.ct[m], p->log2_n, fwd, fixed, sc)
         if (p->log2_n == 9) { if (soft) NHP_XL(true, 9); else NHP_XL(false, 9); }
         else if (p->log2_n == 10) { if (soft) NHP_XL(true, 10); else NHP_XL(false, 10); }
         else { if (soft) NHP_XL(true, 0); else NHP_XL(false, 0); }
@@ -527,8 +547,8 @@ int launch_straight_tile(nhp_planner *p, int m)
     }
     {
         ProfScope py(p, 15);
-        if (soft) straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
-        else straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
+        if (soft) straight_rows_kernel<true><<<gy, warps * 32, 0, p->stream>>>(p->V, p->S_line, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed, sc);
+        else straight_rows_kernel<false><<<gy, warps * 32, 0, p->stream>>>(p->V, nullptr, p->d_B, p->d_IJ, p->d_tlist + nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed, sc);
     }
     return 2;
 }

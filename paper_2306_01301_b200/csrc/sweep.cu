@@ -735,22 +735,26 @@ int launch_cycles(nhp_planner *p, int n_cycles, bool fresh)
         } else if (fwd_only) {
             launches += inner();
         } else {
-            if (c == 0) {
-                // The very first LF of a plan finds one finite vertex, the start: only the left-turn curve through it can change
-                // (PAPER.md:392 step 5; eq (18) inverted gives its thread coordinates), so one tile is launched instead of N^2 / 32.
-                // Not with a maneuver in progress at the start (more seeds) and not in the fixed-work modes.
-                if (fresh && p->start_m0 < 0 && !(p->w.flags & (NHP_FLAG_FIXED_WORK | NHP_FLAG_NO_SHORTCUTS))) {
-                    const int mt = p->nt - 1, mx = p->n - 1, q = p->nt >> 2, th = p->start[2];
-                    const int xp = (p->start[0] - p->beta[th & mt]) & mx, yp = (p->start[1] - p->beta[(th + 3 * q) & mt]) & mx;
-                    launches += launch_turn_tile(p, L, M_LF, -1, xp >> 5, yp);
-                } else launches += launch_turn_tile(p, L, M_LF, -1);
+            // The very first LF of a plan finds one finite vertex, the start: only the left-turn curve through it can change
+            // (PAPER.md:392 step 5; eq (18) inverted gives its thread coordinates), so one tile is launched instead of N^2 / 32; and
+            // the SF that follows finds one finite vertex per Theta plane, those of that curve: one band per slice (streaming
+            // kernels).  Not with a maneuver in progress at the start (more seeds) and not in the fixed-work modes.
+            const bool first_sparse = c == 0 && fresh && p->start_m0 < 0 && !(p->w.flags & (NHP_FLAG_FIXED_WORK | NHP_FLAG_NO_SHORTCUTS));
+            int xp = 0, yp = 0;
+            if (first_sparse) {
+                const int mt = p->nt - 1, mx = p->n - 1, q = p->nt >> 2, th = p->start[2];
+                xp = (p->start[0] - p->beta[th & mt]) & mx; yp = (p->start[1] - p->beta[(th + 3 * q) & mt]) & mx;
             }
-            if (c + 1 < n_cycles) launches += inner();
+            if (c == 0) launches += first_sparse ? launch_turn_tile(p, L, M_LF, -1, xp >> 5, yp) : launch_turn_tile(p, L, M_LF, -1);
+            const bool last = c + 1 == n_cycles;
+            if (!last && !(first_sparse && !graph)) launches += inner();
             else {
+                if (first_sparse && !graph) { p->sparse_xp = xp; p->sparse_yp = yp; }
                 launches += launch_straight(p, M_SF);
+                p->sparse_xp = p->sparse_yp = -1;
                 launches += launch_turn_tile(p, L, M_RB, M_RF);
                 launches += launch_straight(p, M_SB);
-                launches += launch_turn_tile(p, L, M_LB, -1);
+                launches += last ? launch_turn_tile(p, L, M_LB, -1) : launch_turn_tile(p, L, M_LB, M_LF);
             }
         }
     }

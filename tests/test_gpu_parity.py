@@ -535,6 +535,30 @@ def test_no_write_outside_the_buffers_and_run_to_run_identical(mods):
         p.close()
 
 
+def test_first_cycle_with_the_sparse_launches(mods):
+    """The first LF of a plan is launched as one tile and the first SF as one band per slice (sweep.cu: launch_cycles).  On small grids
+    that path is taken only while the CUDA graph of the inner cycle is off, i.e. under per-kernel profiling: parity cycle by cycle
+    there, for several starts, hard and soft."""
+    oracle, nhp = mods
+    for sc in (scenes.random_scene(6, 6, 8, 41, n_rects=8), scenes.random_scene(7, 6, 9, 42, soft=True, reverse_mult=300, vehicle=(6, 3)),
+               scenes.random_scene(5, 7, 4, 43)):
+        o, fp = oracle_for(oracle, sc)
+        Cv, Sv = o.render(fp, sc.hard, sc.soft)
+        p = nhp.Planner.from_scene(sc)
+        p.render_obstacles(sc.hard, sc.soft)
+        p.set_profiling(True)
+        free = np.argwhere(Cv == 0)
+        rng = np.random.default_rng(7)
+        for k in rng.integers(len(free), size=6):
+            start = (int(free[k][2]), int(free[k][1]), int(free[k][0]))
+            for n_cycles in (1, 2):
+                p.run_nturn(start, n_cycles)
+                V = o.run(Cv, Sv, start, n_cycles)
+                got = p.cost_volume_numpy()
+                assert (got == V).all(), (sc.name, start, n_cycles, int((got != V).sum()))
+        p.close()
+
+
 def _full_config(mods, k, sample_render=20000):
     oracle, nhp = mods
     sc = scenes.get_config(k)
