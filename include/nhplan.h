@@ -187,6 +187,42 @@ int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *sof
  * Requires NHP_FLAG_SOFT.  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_CUDA. */
 int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, double k, float *dist_dev_out);
 
+/* Steps 1-2 of PAPER.md:388-389 alone (distance transform + soft image, reading DESIGN R17 exactly as in
+ * nhp_render_obstacles_dt), for callers that are NOT ALLOWED TO ALLOCATE DEVICE MEMORY and so cannot even own a planner
+ * handle (nhp_planner_create calls cudaMalloc for its tables).  Who that is: a planning thread inside a vehicle's control
+ * loop, where the memory budget is fixed and audited at start-up and a cudaMalloc -- which takes a driver-wide lock, may
+ * wait for the whole device to go idle and can fail on a fragmented heap -- has no bounded latency; a plug-in living in a
+ * process whose host framework has already claimed nearly all of HBM for its own pool, so that a raw cudaMalloc simply
+ * fails; code running under a "no allocation after initialisation" rule of a safety process.  This call needs no handle,
+ * calls no cudaMalloc / cudaFree and no library routine that allocates, neither on the device nor on the host.
+ *
+ * The one intermediate image of the transform (per pixel the distance to the nearest obstacle pixel of its column,
+ * int32) lives in an array that is part of the library image itself: NHP_NOALLOC_MAX_N^2 x 4 bytes = 4 MiB of device
+ * memory on EVERY GPU whose context loads libnhplan.so, held until the process exits whether or not this call is ever made.
+ *   hard_dev      DEVICE, n x n uint8, row = y, column = x, non-zero = hard obstacle; row 0 and column 0 count as wall
+ *   n             image side, 1 <= n <= NHP_NOALLOC_MAX_N (any n, not only powers of two).  A larger n is refused with
+ *                 NHP_E_BUFFER and a message that names the limit: the array cannot grow
+ *   k             strength of the soft cost, 0 <= k <= 64, as in nhp_render_obstacles_dt
+ *   soft_dev_out  DEVICE, n x n uint8, receives the Q4.4 soft image (caller-owned, like every input and output)
+ *   dist_dev_out  DEVICE, n x n float32, receives the distances, or NULL
+ *   cuda_stream   a cudaStream_t of the device that owns the three buffers (0 = legacy default stream); the two kernels
+ *                 are enqueued there and the call returns without waiting for them
+ * The device that owns hard_dev is made current for the duration of the call; the outputs must live on the same device.
+ * First call on a device: the library asks the runtime where that device keeps its copy of the array (each device has its
+ * own, at its own address) and remembers the answer; later calls on that device skip this.  Make that first call during
+ * start-up, before any stream capture is begun on the device.
+ * Shared state: ALL calls on a device use the same array -- any stream, any thread -- and it keeps whatever the last
+ * call left in it.  Nothing has to be cleared between calls (each call overwrites the n x n words it is going to read
+ * before it reads them), but two calls whose kernels can run at the same time on one device (different streams without
+ * an ordering between them) overwrite each other's intermediate image and produce garbage: order them yourself.
+ * Errors: NHP_E_ARG (NULL pointer, n < 1, k out of range), NHP_E_BUFFER (n > NHP_NOALLOC_MAX_N; a pointer that is not
+ * plain device memory or lives on another device), NHP_E_CUDA.  nhp_noalloc_last_error() returns the text of the calling
+ * thread's last failure of this entry point ("" after a success; never NULL; static storage). */
+#define NHP_NOALLOC_MAX_N 1024
+int nhp_soft_from_hard_noalloc(const uint8_t *hard_dev, int n, double k, uint8_t *soft_dev_out, float *dist_dev_out,
+                               void *cuda_stream);
+const char *nhp_noalloc_last_error(void);
+
 /* Debug accessor: the soft image the last render used (N x N uint8) -> HOST.  Synchronises the stream. */
 int nhp_debug_soft_image(nhp_planner *p, uint8_t *soft_host);
 

@@ -6,5 +6,5 @@ memory and the stream, nothing else.  There is no CPU fallback: importing `Plann
 library, or constructing one without a CUDA device, raises.
 """
 from .binding import (  # noqa: F401
-    DEFAULT_CYCLES, FLAG_FIXED_WORK, FLAG_FORWARD_ONLY, FLAG_NO_SHORTCUTS, FLAG_SECTIONS, FLAG_NO_SECTIONS, FLAG_SIMPLE_KERNELS, FLAG_SOFT, INF, MANEUVER_NAMES, NhpError, Planner, lib_path, load_library,
+    DEFAULT_CYCLES, FLAG_FIXED_WORK, FLAG_FORWARD_ONLY, FLAG_NO_SHORTCUTS, FLAG_SECTIONS, FLAG_NO_SECTIONS, FLAG_SIMPLE_KERNELS, FLAG_SOFT, INF, MANEUVER_NAMES, NhpError, NOALLOC_MAX_N, Planner, lib_path, load_library, soft_from_hard_noalloc,
 )

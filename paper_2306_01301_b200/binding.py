@@ -21,7 +21,8 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_render_vehicle_footprint", "nhp_set_box", "nhp_render_obstacles", "nhp_render_obstacles_dt", "nhp_debug_soft_image",
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
-           "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu", "nhp_microbench_read")
+           "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu", "nhp_microbench_read",
+           "nhp_soft_from_hard_noalloc", "nhp_noalloc_last_error")
 KERNEL_SLOTS = 17
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
                      "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows", "straight_sect")
@@ -105,6 +106,9 @@ def load_library():
         L.nhp_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_longlong), C.c_int]
         L.nhp_microbench_alu.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
         L.nhp_microbench_read.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        L.nhp_soft_from_hard_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.nhp_noalloc_last_error.argtypes = []
+        L.nhp_noalloc_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -116,6 +120,30 @@ def query_sizes(log2_n, log2_ntheta, flags=0, max_footprint_radius=0, max_reach_
     if rc:
         raise NhpError(rc, "query_sizes")
     return s
+
+
+NOALLOC_MAX_N = 1024                                        # NHP_NOALLOC_MAX_N
+
+
+def soft_from_hard_noalloc(hard, k, soft_out, dist_out=None, stream=None):
+    """nhp_soft_from_hard_noalloc: distance transform + soft image of an n x n obstacle image, n <= NOALLOC_MAX_N, without a
+    planner handle and without any allocation inside the library -- for callers that may not allocate device memory after
+    start-up (control loops with a fixed memory budget, guests of a process whose pool already owns the GPU's memory).
+    The caller brings every buffer: `hard` (uint8, n x n), `soft_out` (uint8, n x n) and optionally `dist_out` (float32,
+    n x n), all contiguous CUDA tensors on one device; `stream` is a torch stream of that device (default: its current one).
+    The work is enqueued, not waited for.  All calls on a device share one built-in scratch image: calls that could overlap on
+    the GPU must be ordered by the caller (include/nhplan.h has the full contract)."""
+    import torch
+    L = load_library()
+    n = hard.shape[0]
+    for t, dt in ((hard, torch.uint8), (soft_out, torch.uint8), (dist_out, torch.float32)):
+        if t is not None:
+            assert t.is_cuda and t.dtype == dt and t.is_contiguous() and tuple(t.shape) == (n, n)
+    st = stream if stream is not None else torch.cuda.current_stream(hard.device)
+    rc = L.nhp_soft_from_hard_noalloc(hard.data_ptr(), int(n), float(k), soft_out.data_ptr(),
+                                      dist_out.data_ptr() if dist_out is not None else None, C.c_void_p(st.cuda_stream))
+    if rc:
+        raise NhpError(rc, f"soft_from_hard_noalloc: {L.nhp_noalloc_last_error().decode()}")
 
 
 class Planner:
