@@ -394,7 +394,8 @@ def run_ours(args):
                 "frac": alu_achieved / alu_peak, "ops_per_pose_update": ops_per_update,
                 "peak_source": f"nhp_microbench_alu, measured in this run: 8 independent VIADDMNMX chains per thread, 8 warps per sub-partition, "
                                f"{sm_count} SMs = {alu_ops / (sm_count * 4 * sm_clock * 1e6):.2f} lane-ops per sub-partition and clock at {sm_clock:.0f} MHz (DESIGN.md 6.7)"},
-        "read_probe_gbs": {name: p.microbench_read(k) / 1e9 for k, name in enumerate(("linear", "rows_pattern", "xrows_pattern", "turn_tile_pattern"))},
+        "read_probe_gbs": {name: (p.microbench_read(k) / 1e9 if k < 3 or p.nt <= 1024 else None)       # the turn-tile pattern is one CTA of N_theta threads
+                           for k, name in enumerate(("linear", "rows_pattern", "xrows_pattern", "turn_tile_pattern"))},
         "kernel_ms_per_step": {k: round(v[0] / args.steps, 4) for k, v in top_level.items()},
         "kernel_ms_sum": sum(v[0] for v in top_level.values()) / args.steps,
         "ms_per_step_with_kernel_events": step_prof_ms,

@@ -29,6 +29,9 @@
  * vertices read NHP_INF in the exported volume.
  *
  * Thread safety: one handle <-> one stream <-> one caller thread at a time.
+ * Memory kinds: the nhp_buffers must be plain device memory (cudaMalloc or a pool built on it) of ONE device; managed
+ * (cudaMallocManaged) and host-mapped memory are refused at create with NHP_E_BUFFER, as are buffers on different devices.
+ * The stream must belong to that device (not checked).
  */
 #ifndef NHPLAN_H
 #define NHPLAN_H
@@ -318,6 +321,11 @@ int nhp_debug_tables(const nhp_planner *p, int32_t *beta, uint8_t *psi2, int32_t
  *   cap       bytes available at `covered`
  * Synchronises the stream.  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_BUFFER, NHP_E_CUDA. */
 int nhp_debug_footprint(nhp_planner *p, int *radius, uint8_t *covered, size_t cap);
+
+/* Debug setter: how many waypoints of a plan come back in the same device-to-host copy as the status words (default 128; a
+ * longer plan takes a second copy).  Tests set it to a small number to exercise the second copy with short plans.
+ * 1 <= n_waypoints <= 4096.  Errors: NHP_E_ARG. */
+int nhp_debug_set_plan_eager(nhp_planner *p, int n_waypoints);
 
 /* Number of kernels launched by this handle since creation (for bench.py's gpu_launches). */
 long long nhp_launch_count(const nhp_planner *p);

@@ -203,8 +203,6 @@ int fetch_plan(nhp_planner *p, const int32_t *d_st)
 
 }  // namespace
 
-int set_kernel_attributes(nhp_planner *p);     // straight.cu: per-device function attributes, set at creation
-
 bool prof_grow(nhp_planner *p)
 {
     const size_t pairs = p->ev.size() / 2;
@@ -259,6 +257,14 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
         return NHP_E_BUFFER;
     }
     p->device = attr.device;
+    for (const void *b : {(const void *)dev->C, (const void *)p->S, (const void *)dev->workspace}) {       // one device owns them all
+        cudaPointerAttributes a{};
+        if (b && (cudaPointerGetAttributes(&a, b) != cudaSuccess || a.type != cudaMemoryTypeDevice || a.device != p->device)) {
+            cudaGetLastError();
+            delete p;
+            return NHP_E_BUFFER;
+        }
+    }
     DeviceGuard guard(p);
     // carve the workspace
     const WsLayout L = workspace_layout(log2_n, log2_ntheta, w->flags, lim);
@@ -278,10 +284,6 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     if (rc == NHP_OK) rc = upload_tables(p);
     const size_t npx = (size_t)p->n * p->n;
     p->plan_cap = NHP_PLAN_CAP;
-    if (const char *e = std::getenv("NHP_PLAN_EAGER")) {                 // test knob: exercise the second copy with short plans
-        const int v = std::atoi(e);
-        if (v >= 1 && v <= NHP_PLAN_CAP) p->plan_eager = v;
-    }
     const size_t sp_bytes = sizeof(int32_t) * NHP_STATUS_WORDS + sizeof(nhp_waypoint) * p->plan_cap;      // status words + plan
     auto alloc = [&](void **ptr, size_t bytes) { if (rc == NHP_OK && cudaMalloc(ptr, bytes) != cudaSuccess) rc = NHP_E_CUDA; };
     alloc((void **)&p->d_hard, npx);
@@ -393,6 +395,14 @@ int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, 
     p->have_render = true;
     p->have_run = false;
     p->r_n_levels = -1;
+    return NHP_OK;
+}
+
+int nhp_debug_set_plan_eager(nhp_planner *p, int n_waypoints)
+{
+    if (!p) return NHP_E_ARG;
+    if (n_waypoints < 1 || n_waypoints > NHP_PLAN_CAP) return fail(p, NHP_E_ARG, "n_waypoints outside [1, plan capacity]");
+    p->plan_eager = n_waypoints;
     return NHP_OK;
 }
 

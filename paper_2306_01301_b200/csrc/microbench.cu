@@ -4,12 +4,17 @@
 // thread, 8 warps per SM sub-partition, and is timed with CUDA events on the handle's stream.
 #include "nhp_internal.cuh"
 
+// The probes' own sink word (device code names it directly): written only if an impossible value turns up, which keeps the
+// measured instructions alive without touching anything of the planner's.
+#pragma nv_diag_suppress 550                      /* "set but never used": that is the point of a sink */
+static __device__ uint32_t probe_sink;
+
 namespace {
 
 constexpr int MB_ITERS = 4096, MB_THREADS = 256, MB_CTAS_PER_SM = 4;
 
 template <int CH>
-__global__ void __launch_bounds__(MB_THREADS) alu_chain_kernel(uint32_t *__restrict__ sink, uint32_t w, uint32_t u)
+__global__ void __launch_bounds__(MB_THREADS) alu_chain_kernel(uint32_t w, uint32_t u)
 {
     uint32_t t[CH];
 #pragma unroll
@@ -25,13 +30,13 @@ __global__ void __launch_bounds__(MB_THREADS) alu_chain_kernel(uint32_t *__restr
     uint32_t x = 0;
 #pragma unroll
     for (int c = 0; c < CH; c++) x ^= t[c];
-    if (x == 0xdeadbeefu) sink[0] = x;                // keeps the chains alive; never true for the arguments passed
+    if (x == 0xdeadbeefu) probe_sink = x;               // keeps the chains alive; never true for the arguments passed
 }
 
 template <int CH>
-void launch(int ctas, uint32_t *sink, cudaStream_t s)
+void launch(int ctas, cudaStream_t s)
 {
-    alu_chain_kernel<CH><<<ctas, MB_THREADS, 0, s>>>(sink, 3u, 0x7fff0000u);
+    alu_chain_kernel<CH><<<ctas, MB_THREADS, 0, s>>>(3u, 0x7fff0000u);
 }
 
 }  // namespace
@@ -43,21 +48,20 @@ extern "C" int nhp_microbench_alu(nhp_planner *p, int chains, double *lane_ops_p
     int n_sm = 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess) return NHP_E_CUDA;
     const int ctas = n_sm * MB_CTAS_PER_SM;
-    uint32_t *sink = (uint32_t *)p->d_status + NHP_STATUS_WORDS - 1;       // never written (see the kernel)
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NHP_E_CUDA;
     float best = 1e30f;
     for (int rep = 0; rep < 4; rep++) {                                  // first repetition warms up
         cudaEventRecord(e0, p->stream);
         switch (chains) {
-            case 1: launch<1>(ctas, sink, p->stream); break;
-            case 2: launch<2>(ctas, sink, p->stream); break;
-            case 3: launch<3>(ctas, sink, p->stream); break;
-            case 4: launch<4>(ctas, sink, p->stream); break;
-            case 5: launch<5>(ctas, sink, p->stream); break;
-            case 6: launch<6>(ctas, sink, p->stream); break;
-            case 7: launch<7>(ctas, sink, p->stream); break;
-            default: launch<8>(ctas, sink, p->stream); break;
+            case 1: launch<1>(ctas, p->stream); break;
+            case 2: launch<2>(ctas, p->stream); break;
+            case 3: launch<3>(ctas, p->stream); break;
+            case 4: launch<4>(ctas, p->stream); break;
+            case 5: launch<5>(ctas, p->stream); break;
+            case 6: launch<6>(ctas, p->stream); break;
+            case 7: launch<7>(ctas, p->stream); break;
+            default: launch<8>(ctas, p->stream); break;
         }
         cudaEventRecord(e1, p->stream);
         if (cudaEventSynchronize(e1) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return NHP_E_CUDA; }
@@ -83,7 +87,7 @@ extern "C" int nhp_microbench_alu(nhp_planner *p, int chains, double *lane_ops_p
 //   pattern 3  turn-like (turn_tile_kernel): CTA = N_theta / 32 warps, warp s reads planes 32 s .. 32 s + 31 of one tile
 // ---------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void read_probe_kernel(const uint32_t *__restrict__ V, uint32_t *__restrict__ sink, int log2_n, int nt)
+__global__ void read_probe_kernel(const uint32_t *__restrict__ V, int log2_n, int nt)
 {
     const int lane = threadIdx.x & 31, n = 1 << log2_n, NT = n >> 5;
     const size_t gw = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -102,7 +106,7 @@ __global__ void read_probe_kernel(const uint32_t *__restrict__ V, uint32_t *__re
 #pragma unroll
         for (int k = 0; k < 32; k++) acc ^= u[k];
     }
-    if (acc == 0x12345678u) sink[0] = acc;              // keeps the loads alive; a volume of costs never XORs to this in every thread
+    if (acc == 0x12345678u) probe_sink = acc;             // keeps the loads alive; a volume of costs never XORs to this in every thread
 }
 
 extern "C" int nhp_microbench_read(nhp_planner *p, int pattern, double *bytes_per_s)
@@ -114,17 +118,16 @@ extern "C" int nhp_microbench_read(nhp_planner *p, int pattern, double *bytes_pe
     const int threads = pattern == 3 ? nt : 128;
     const unsigned blocks = (unsigned)(warps * 32 / threads);
     if (pattern == 3 && nt > 1024) return NHP_E_ARG;
-    uint32_t *sink = (uint32_t *)p->d_status + NHP_STATUS_WORDS - 1;
     cudaEvent_t e0, e1;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return NHP_E_CUDA;
     float best = 1e30f;
     for (int rep = 0; rep < 4; rep++) {
         cudaEventRecord(e0, p->stream);
         switch (pattern) {
-            case 0: read_probe_kernel<0><<<blocks, threads, 0, p->stream>>>(p->V, sink, p->log2_n, nt); break;
-            case 1: read_probe_kernel<1><<<blocks, threads, 0, p->stream>>>(p->V, sink, p->log2_n, nt); break;
-            case 2: read_probe_kernel<2><<<blocks, threads, 0, p->stream>>>(p->V, sink, p->log2_n, nt); break;
-            default: read_probe_kernel<3><<<blocks, threads, 0, p->stream>>>(p->V, sink, p->log2_n, nt); break;
+            case 0: read_probe_kernel<0><<<blocks, threads, 0, p->stream>>>(p->V, p->log2_n, nt); break;
+            case 1: read_probe_kernel<1><<<blocks, threads, 0, p->stream>>>(p->V, p->log2_n, nt); break;
+            case 2: read_probe_kernel<2><<<blocks, threads, 0, p->stream>>>(p->V, p->log2_n, nt); break;
+            default: read_probe_kernel<3><<<blocks, threads, 0, p->stream>>>(p->V, p->log2_n, nt); break;
         }
         cudaEventRecord(e1, p->stream);
         if (cudaEventSynchronize(e1) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return NHP_E_CUDA; }

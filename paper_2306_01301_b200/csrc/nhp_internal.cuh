@@ -113,8 +113,8 @@ struct nhp_planner {
     uint8_t *d_Mk = nullptr;       // [levels][n][n]    soft image; level k = max over 2^k columns (soft only)
     bool have_render = false, have_run = false, canonical = false;
     int start[3] = {0, 0, 0};
-    // reachability (bit-vector) planner, reach.cu: level volumes and the transposed working volumes (allocated at the first
-    // nhp_reach_run), number of levels of the last run, its start
+    // reachability (bit-vector) planner, reach.cu: level volumes and the transposed working volumes (carved from the caller's
+    // workspace at create), number of levels of the last run, its start
     uint32_t *r_levels = nullptr, *r_Lt = nullptr, *r_Ct = nullptr, *r_Gt = nullptr;   // in the caller's workspace
     int r_n_levels = -1, r_start[3] = {0, 0, 0};
     int sparse_xp = -1, sparse_yp = -1;   // >= 0 only while launch_cycles launches the first SF of a plan (straight.cu: StartCurve)

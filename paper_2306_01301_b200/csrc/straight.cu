@@ -532,10 +532,9 @@ int launch_straight_tile(nhp_planner *p, int m)
         if (soft) straight_sect_kernel<true><<<dim3(bands, nt), bands * 32, smx, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, p->d_tlist, nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
         else straight_sect_kernel<false><<<dim3(bands, nt), bands * 32, smx, p->stream>>>(p->V, p->S_line, p->d_B, p->d_xl_tab, p->d_IJ, p->d_tlist, nx, lenq, p->w.ct[m], p->log2_n, fwd, fixed);
         return 1;
-        return 2;
     }
     {
-        const int xw = bands < XL_WARPS_V ? bands : XL_WARPS_V;
+        const int xw = sparse ? 1 : bands < XL_WARPS_V ? bands : XL_WARPS_V;      // sparse: the one band that holds the line, one warp
         const size_t smem = sizeof(uint32_t) * (size_t)xw * XL_STAGE;
         const dim3 gx(sparse ? 1 : bands / xw, nx);
         ProfScope px(p, 14);

@@ -316,7 +316,7 @@ def test_no_device_allocation_after_create(mods):
     p.close()
 
 
-def test_default_cycles_and_long_plans(mods, monkeypatch):
+def test_default_cycles_and_long_plans(mods):
     """n_cycles <= 0 selects the paper's default of 8 cycles; a plan longer than the waypoints that travel with
     the status words comes back complete (second copy)."""
     oracle, nhp = mods
@@ -324,8 +324,8 @@ def test_default_cycles_and_long_plans(mods, monkeypatch):
     o, fp = oracle_for(oracle, sc)
     Cv, _ = o.render(fp, sc.hard, None, method="brute")
     V = o.run(Cv, None, sc.start, 8)
-    monkeypatch.setenv("NHP_PLAN_EAGER", "2")
     p = nhp.Planner.from_scene(sc)
+    p.debug_set_plan_eager(2)
     p.render_obstacles(sc.hard)
     p.run_nturn(sc.start, 0)
     assert (p.cost_volume_numpy() == V).all()
