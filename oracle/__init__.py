@@ -70,6 +70,7 @@ def _load():
         L.orc_render_pose.argtypes = [C.c_void_p, C.POINTER(_Footprint), C.c_void_p, C.c_void_p,
                                       C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_render_brute.argtypes = [C.c_void_p, C.POINTER(_Footprint)] + [C.c_void_p] * 4
+        L.orc_render_brute_plane.argtypes = [C.c_void_p, C.POINTER(_Footprint), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_render_runs.argtypes = [C.c_void_p, C.POINTER(_Footprint)] + [C.c_void_p] * 4
         L.orc_footprint_offsets.argtypes = [C.c_void_p, C.POINTER(_Footprint), C.c_int, C.c_void_p, C.c_void_p, C.c_int]
         L.orc_sweep.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -199,6 +200,16 @@ class Oracle:
         if rc:
             raise OracleError(rc, "render")
         return Cv, Sv
+
+    def render_plane(self, fp: Footprint, hard, soft, t):
+        """Plane t of the brute-force rendering -> (C uint8 [j][i], S uint8 or None)."""
+        hard, soft = self._imgs(hard, soft)
+        Cp = np.empty((self.n, self.n), np.uint8)
+        Sp = np.empty((self.n, self.n), np.uint8) if soft is not None else None
+        rc = _load().orc_render_brute_plane(self._h, C.byref(fp._c), _ptr(hard), _ptr(soft), int(t), _ptr(Cp), _ptr(Sp))
+        if rc:
+            raise OracleError(rc, "render_plane")
+        return Cp, Sp
 
     def footprint_offsets(self, fp: Footprint, t):
         cap = (2 * fp.radius() + 1) ** 2

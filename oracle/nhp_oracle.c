@@ -314,6 +314,24 @@ int orc_render_brute(const orc_ctx *c, const orc_footprint *fp, const uint8_t *h
     return 0;
 }
 
+/* One Theta plane of orc_render_brute: the same per-pose definition (orc_render_pose) over all (i, j) of plane t and nothing
+ * else, for whole-plane checks at sizes where the full brute-force volume takes too long.  C_out / S_out: n x n. */
+int orc_render_brute_plane(const orc_ctx *c, const orc_footprint *fp, const uint8_t *hard, const uint8_t *soft, int t,
+                           uint8_t *C_out, uint8_t *S_out)
+{
+    int n = c->n;
+    if (2 * orc_footprint_radius(fp) >= n || t < 0 || t >= c->nt) return -1;
+#pragma omp parallel for num_threads(c->threads) schedule(static)
+    for (int j = 0; j < n; j++)
+        for (int i = 0; i < n; i++) {
+            uint8_t cc, ss;
+            orc_render_pose(c, fp, hard, soft, i, j, t, &cc, &ss);
+            C_out[(size_t)j * n + i] = cc;
+            if (S_out) S_out[(size_t)j * n + i] = soft ? ss : 16;
+        }
+    return 0;
+}
+
 /* Number of covered offsets for Theta (area check) and optional list output. */
 int orc_footprint_offsets(const orc_ctx *c, const orc_footprint *fp, int t, int32_t *da_out, int32_t *db_out, int cap)
 {

@@ -113,6 +113,10 @@ def test_run_renderer_equals_brute_force(seed, vehicle, soft):
         i, j, t = (int(rng.integers(o.n)), int(rng.integers(o.n)), int(rng.integers(o.nt)))
         c, s = o.render_pose(fp2, sc.hard, sc.soft, i, j, t)
         assert c == Cb[t, j, i] and (Sb is None or s == Sb[t, j, i])
+    # ... and so do single planes (the form the full-size GPU tests use)
+    for t in (0, o.nt // 8, o.nt - 3):
+        Cp, Sp = o.render_plane(fp2, sc.hard, sc.soft, t)
+        assert (Cp == Cb[t]).all() and (Sb is None or (Sp == Sb[t]).all())
 
 
 def test_run_renderer_equals_brute_force_with_a_large_footprint():
