@@ -60,19 +60,48 @@ def workload_name(sc, n_cycles):
             f"N_T={n_cycles}, {'soft+hard' if sc.soft is not None else 'hard'} obstacles")
 
 
-def measured_traffic(config, slot):
-    """dram bytes per launch of `slot` from the committed ncu capture (profiles/traffic.csv), or None."""
+SLOT_SOURCES = {"straight_xrows": "straight.cu", "straight_rows": "straight.cu", "straight_sect": "straight.cu", "SF": "straight.cu", "SB": "straight.cu",
+                "render_collision": "render.cu", "render_soft": "render.cu", "backtrack": "backtrack.cu", "distance_transform": "distance.cu"}     # default: sweep.cu
+
+
+def source_hashes():
+    """sha256 (first 16 hex digits) of every kernel source: a committed ncu byte count is only divided by a fresh time when the
+    kernel's source (and the shared header) is still the one the capture was taken from."""
+    import glob
+    import hashlib
+    d = os.path.join(ROOT, "paper_2306_01301_b200", "csrc")
+    return {os.path.basename(p): hashlib.sha256(open(p, "rb").read()).hexdigest()[:16] for p in sorted(glob.glob(os.path.join(d, "*.cu*")))}
+
+
+def traffic_table():
+    """profiles/traffic.csv -> ({(config, slot): (bytes, source)}, {file: sha16 at capture}, commit the captures were taken at)."""
+    rows, hashes, commit = {}, {}, None
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for ln in f:
-                if ln.startswith("#") or not ln.strip():
-                    continue
-                c, k, b, src = ln.strip().split(",", 3)
-                if c == str(config) and k == slot:
-                    return {"bytes_per_launch": int(b), "source": src}
+                ln = ln.strip()
+                if ln.startswith("# sha16 "):
+                    hashes = dict(kv.split("=") for kv in ln[8:].split())
+                elif ln.startswith("# commit "):
+                    commit = ln[9:].strip()
+                elif ln and not ln.startswith("#"):
+                    c, k, b, src = ln.split(",", 3)
+                    rows[(c, k)] = (int(b), src)
     except OSError:
         pass
-    return None
+    return rows, hashes, commit
+
+
+def measured_traffic(config, slot):
+    """dram bytes per launch of `slot` from the committed ncu capture (profiles/traffic.csv), or None.  `stale` = the kernel's
+    source or the shared header changed since the capture: the bytes are shown, frac_traffic is not computed from them."""
+    rows, hashes, _ = traffic_table()
+    if (str(config), slot) not in rows:
+        return None
+    now = source_hashes()
+    files = (SLOT_SOURCES.get(slot, "sweep.cu"), "nhp_internal.cuh")
+    b, src = rows[(str(config), slot)]
+    return {"bytes_per_launch": b, "source": src, "stale": any(hashes.get(fn) != now.get(fn) for fn in files)}
 
 
 def peak_hbm():
@@ -230,6 +259,17 @@ class PlanBench:
         kt = p.kernel_times(reset=True) if profile else None
         return e0.elapsed_time(e1), p.launch_count() - l0, kt
 
+    def launch_path(self):
+        """Which launch sequence the timed pass and the event-bracketed (profiled) pass run (they differ on small grids)."""
+        if self.reach:
+            return {"timed": "separate launches", "profiled": "separate launches"}
+        fl, nhp = self.p.flags, self.nhp
+        sparse = not fl & (nhp.FLAG_FIXED_WORK | nhp.FLAG_NO_SHORTCUTS | nhp.FLAG_SIMPLE_KERNELS | nhp.FLAG_FORWARD_ONLY)
+        first = "one-tile first LF" if sparse else "full first LF"
+        sep = f"separate launches, {first}, " + ("one-band first SF" if sparse else "full first SF")
+        g = self.p.cycle_graph_kernels()
+        return {"timed": f"CUDA graph of the inner cycle ({g} kernels per replay), {first}, full first SF" if g else sep, "profiled": sep}
+
     def updates_per_launch(self, slot):
         """Pose-updates one launch of `slot` processes (N_R per maneuver kernel)."""
         nt = self.sc.nt
@@ -237,8 +277,9 @@ class PlanBench:
                 "straight_rows": self.n_r * (nt - self.nx) // nt}.get(slot, self.n_r)
 
     def rooflines(self, kt, steps, step_ms, peak, config):
-        """Per sweep kernel: algorithmic bytes / CUDA-event time (`frac`, the 6-pass definition of SURVEY 8(d)) and the
-        committed ncu dram bytes / the same time (`frac_traffic`, the physical HBM fraction)."""
+        """Per sweep kernel: algorithmic bytes / CUDA-event time (`frac_nominal`, the 6-pass definition of SURVEY 8(d): NOT a
+        physical fraction while the short cuts are on) and the committed ncu dram bytes / the same time (`frac_traffic`, the
+        physical HBM fraction)."""
         alg_b = ALG_BYTES_SOFT if self.sc.soft is not None else ALG_BYTES_HARD
         out = {}
         for k in SWEEP_SLOTS:
@@ -251,11 +292,13 @@ class PlanBench:
             alg = alg_b * self.updates_per_launch(k)
             tr = measured_traffic(config, k)
             ach = alg / (avg * 1e-3) / 1e9
+            fresh = tr is not None and not tr["stale"]
             out[k] = {"avg_launch_ms": avg, "launches_timed": int(n), "ms_per_step": ms / steps, "share_of_step": ms / steps / step_ms,
                       "pose_updates_per_launch": self.updates_per_launch(k), "algorithmic_bytes_per_launch": alg,
-                      "achieved": ach, "frac": ach / peak,
+                      "achieved_nominal": ach, "frac_nominal": ach / peak,
                       "traffic": tr["bytes_per_launch"] if tr else None, "traffic_source": tr["source"] if tr else None,
-                      "frac_traffic": (tr["bytes_per_launch"] / (avg * 1e-3) / 1e9 / peak) if tr else None}
+                      "traffic_stale": tr["stale"] if tr else None,
+                      "frac_traffic": (tr["bytes_per_launch"] / (avg * 1e-3) / 1e9 / peak) if fresh else None}
         return out
 
     def close(self):
@@ -278,7 +321,8 @@ def side_config(nhp, torch, replicas, dev, config, peak, flags=0, steps=2, cycle
            "value": steps * b.updates_per_plan / (ms * 1e-3) / 1e9, "unit": UNIT, "plans_per_sec": steps / (ms * 1e-3),
            "gpu_launches": int(launches), "plan_waypoints": len(b.plan[0]), "plan_cost": b.plan[1],
            "dominant_kernel": dom,
-           "kernels": {k: {kk: v[kk] for kk in ("avg_launch_ms", "ms_per_step", "frac", "traffic", "frac_traffic")} for k, v in rl.items()},
+           "launch_path": b.launch_path(),
+           "kernels": {k: {kk: v[kk] for kk in ("avg_launch_ms", "ms_per_step", "frac_nominal", "traffic", "traffic_stale", "frac_traffic")} for k, v in rl.items()},
            "kernel_ms_per_step": {k: round(v[0] / steps, 4) for k, v in kt.items() if v[1] and k not in nhp.binding.NESTED_SLOTS}}
     b.close()
     return out
@@ -356,7 +400,7 @@ def run_ours(args):
     sweep_gbs = alg_b * n_r * 6 * n_cycles * args.steps / (sweep_ms * 1e-3) / 1e9 if sweep_ms > 0 else 0.0
     dom_rl = rl.get(dom, {})
     # physical HBM fraction of all sweeps together: committed ncu dram bytes per launch x launches / their summed time
-    tr_known = [k for k in rl if rl[k]["traffic"] is not None]
+    tr_known = [k for k in rl if rl[k]["frac_traffic"] is not None]          # captured, and the kernel's source unchanged since
     tr_bytes = sum(rl[k]["traffic"] * rl[k]["launches_timed"] for k in tr_known)
     tr_ms = sum(sweeps[k][0] for k in tr_known)
     # secondary bound: the integer min/max pipe, measured live by the library's micro-benchmark
@@ -370,20 +414,33 @@ def run_ours(args):
         "metric": METRIC, "value": units / (ms_dev_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": ws,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_dev_max / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32", "data": "synthetic",
+        "value_definition": ("NOMINAL pose-updates (6 * N_T * N_R per plan, PAPER.md:453) / time" +
+                             ("; every data-dependent short cut is off in this run" if (args.fixed_work or args.no_shortcuts or args.simple_kernels) else
+                              ", data-dependent short cuts ON: tiles without a finite value or fully blocked are skipped, a vertex is stored only "
+                              "where it improved, the first LF / SF of a plan touch one tile / one band per slice -- the time depends on the "
+                              "scene; the scene-independent figures are fixed_work_* (same instructions and bytes whatever the scene holds, "
+                              "PAPER.md:565) and no_shortcuts_*")),
+        "launch_path": b.launch_path(),
         "config": bench_config(sc, n_cycles, args, ws, dt_dev),
         "result": {"goal": list(b.goal), "plan_waypoints": len(plan), "plan_cost": cost},
         "plans_per_sec": ws * args.steps / (ms_dev_max * 1e-3),
         "clocks": clk,
         "e2e": {"value": units / (ms_e2e_max * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ms_e2e_max / args.steps,
                 "h2d_bytes_per_step": int(hard_h.numel() + (soft_h.numel() if (soft_h is not None and not dt_dev) else 0)),
-                "d2h_bytes_per_step": int(4 * 16 + 16 * max(len(plan), 128))},
+                "d2h_bytes_per_step": int(4 * 16 + 16 * max(len(plan), nhp.binding.PLAN_EAGER))},      # status words + the waypoints that travel with them
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "kernel": dom, "pose_updates_per_launch": dom_upd, "achieved": achieved, "peak": peak, "unit": "GB/s",
                      "frac": achieved / peak, "traffic": dom_rl.get("traffic"), "frac_traffic": dom_rl.get("frac_traffic"),
                      "traffic_source": dom_rl.get("traffic_source"), "peak_source": peak_src,
-                     "frac_definition": "frac = SURVEY 8(d) algorithmic bytes (8.125 B, 9.125 B soft, per pose-update; a fused pair launch is charged "
-                                        "two maneuvers) / CUDA-event time / peak: above 1 because one read of V serves up to four laps; "
-                                        "frac_traffic = ncu dram bytes per launch (profiles/traffic.csv) / the same time / peak: the physical HBM fraction",
+                     "frac_definition": "frac = SURVEY 8(d) algorithmic bytes (8.125 B, 9.125 B soft, per NOMINAL pose-update; a fused pair launch is "
+                                        "charged two maneuvers) / CUDA-event time / peak.  It is the contract's 6-pass figure, not a physical fraction: it "
+                                        "exceeds 1 because the kernels move fewer bytes than the definition charges -- in every kernel the 4-byte write "
+                                        "happens only where a vertex improved and tiles with nothing to do are skipped (this alone puts the straight "
+                                        "kernels, which fuse nothing, above 1), the collision bit is stamped into V (no separate read), and a turn-pair "
+                                        "launch reads V once for the four laps of two maneuvers.  frac_traffic = ncu dram bytes per launch "
+                                        "(profiles/traffic.csv, captured at traffic_commit; null when the kernel's source changed since) / the same "
+                                        "time / peak: the physical HBM fraction.  Per-kernel rows carry the 6-pass figure as frac_nominal.",
+                     "traffic_commit": traffic_table()[2], "traffic_stale": dom_rl.get("traffic_stale"),
                      "algorithmic_bytes_per_launch": per_launch_bytes, "avg_launch_ms": dom_ms / max(dom_n, 1),
                      "launches_timed": int(dom_n), "launches_untimed": int(dropped),
                      "kernels": rl,
@@ -401,16 +458,39 @@ def run_ours(args):
         "ms_per_step_with_kernel_events": step_prof_ms,
     }
     b.close()
+    rf = out["roofline"]
+    rf["frac_traffic_all_sweeps"] = rf["all_sweeps"]["frac_traffic"]          # scalar copies: the driver's record keeps scalars only
+    rf["traffic_per_step"] = rf["all_sweeps"]["traffic_per_step"]
     if ws == 1 and not args.no_extra:
         # T12 ("run time independent of scene"): the same workload with the data-dependent short cuts off
         if not args.fixed_work and not args.no_shortcuts and not args.simple_kernels:
             for key, fl, cfgkey in (("no_shortcuts", nhp.FLAG_NO_SHORTCUTS, f"{args.config}:no_shortcuts"), ("fixed_work", nhp.FLAG_FIXED_WORK, f"{args.config}:fixed_work")):
                 fw = side_config(nhp, torch, replicas, dev, args.config, peak, flags=fl, steps=min(args.steps, 3), cycles=args.cycles, traffic_key=cfgkey)
                 out[key] = {k: fw[k] for k in ("ms_per_step", "value", "unit", "plans_per_sec", "steps", "kernels")}
+                out[f"{key}_ms_per_step"] = rf[f"{key}_ms_per_step"] = fw["ms_per_step"]
+                out[f"{key}_value"] = fw["value"]
+                # whole plan against the 6-pass definition: with NHP_FLAG_FIXED_WORK the definition's bytes are (at least) moved
+                rf[f"{key}_frac"] = alg_b * 6 * n_cycles * n_r / (fw["ms_per_step"] * 1e-3) / 1e9 / peak
+                kn = fw["kernels"]
+                known = [k for k in kn if kn[k]["frac_traffic"] is not None]
+                t_ms = sum(kn[k]["ms_per_step"] for k in known)
+                rf[f"{key}_frac_traffic_all_sweeps"] = (sum(kn[k]["frac_traffic"] * kn[k]["ms_per_step"] for k in known) / t_ms) if known else None
             out["no_shortcuts"]["what"] = "NHP_FLAG_NO_SHORTCUTS: every warp runs every pass of every sweep; vertices written only where they improved"
             out["fixed_work"]["what"] = "NHP_FLAG_FIXED_WORK: no short cuts and every visited vertex written back (the paper's unconditional store): same instructions and bytes whatever the scene holds"
-        # the soft-cost path and the largest grid, one short timed run each (BASELINE.json configs 4 and 5)
-        out["other_configs"] = [side_config(nhp, torch, replicas, dev, c, peak, steps=2) for c in (4, 5) if c != args.config]
+        # the other configurations of BASELINE.json (small grids, the soft-cost path, the largest grid), one short timed run each
+        out["other_configs"] = [side_config(nhp, torch, replicas, dev, c, peak, steps=2 if c > 2 else 20) for c in (1, 2, 4, 5) if c != args.config]
+        for oc in out["other_configs"]:
+            rf[f"cfg{oc['baseline_config']}_ms_per_step"] = oc["ms_per_step"]
+            dk = oc["kernels"].get(oc["dominant_kernel"] or "", {})
+            rf[f"cfg{oc['baseline_config']}_frac_traffic"] = dk.get("frac_traffic")
+        # the reachability planner of appendix C on the same workload (Table 9)
+        rb = PlanBench(nhp, torch, replicas, scenes.CONFIGS[args.config](replicas.replica_seed(args.config, 0)), n_cycles, dev, reach=True)
+        rb.warm_up(1)
+        r_ms, r_launches, _ = rb.timed(3)
+        out["reach"] = {"what": f"reachability (bit-vector) planner, appendix C: render + {n_cycles} levels + back-track on config {args.config}",
+                        "ms_per_step": r_ms / 3, "steps": 3, "gpu_launches": int(r_launches), "plan_waypoints": len(rb.plan[0]), "plan_maneuvers": rb.plan[1]}
+        rf["reach_ms_per_step"] = out["reach_ms_per_step"] = r_ms / 3
+        rb.close()
     if not args.no_cpu_baseline and ws == 1:
         out["cpu_baseline"] = cpu_baseline(sc, n_cycles, sample_cycles=2)
     replicas.shutdown()

@@ -327,6 +327,10 @@ int nhp_debug_footprint(nhp_planner *p, int *radius, uint8_t *covered, size_t ca
  * 1 <= n_waypoints <= 4096.  Errors: NHP_E_ARG. */
 int nhp_debug_set_plan_eager(nhp_planner *p, int n_waypoints);
 
+/* Debug accessor: number of kernels in the CUDA graph of one inner maneuver cycle that nhp_run_nturn replays while profiling is
+ * off (grids of at most 2^26 poses with the tile kernels), 0 if the handle launches every kernel separately. */
+int nhp_debug_cycle_graph_kernels(const nhp_planner *p);
+
 /* Number of kernels launched by this handle since creation (for bench.py's gpu_launches). */
 long long nhp_launch_count(const nhp_planner *p);
 

@@ -22,7 +22,7 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu", "nhp_microbench_read",
-           "nhp_soft_from_hard_noalloc", "nhp_noalloc_last_error", "nhp_debug_set_plan_eager")
+           "nhp_soft_from_hard_noalloc", "nhp_noalloc_last_error", "nhp_debug_set_plan_eager", "nhp_debug_cycle_graph_kernels")
 KERNEL_SLOTS = 17
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
                      "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows", "straight_sect")
@@ -82,6 +82,7 @@ def load_library():
         L.nhp_render_obstacles_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
         L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
         L.nhp_debug_set_plan_eager.argtypes = [C.c_void_p, C.c_int]
+        L.nhp_debug_cycle_graph_kernels.argtypes = [C.c_void_p]
         L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
         L.nhp_run_nturn_from.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
         L.nhp_reach_run.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
@@ -273,6 +274,10 @@ class Planner:
 
     def run_nturn(self, start, n_cycles=DEFAULT_CYCLES):
         self._check(self._L.nhp_run_nturn(self._h, int(start[0]), int(start[1]), int(start[2]), int(n_cycles)), "run_nturn")
+
+    def cycle_graph_kernels(self):
+        """Kernels in the CUDA graph of one inner cycle that run_nturn replays while profiling is off; 0 = separate launches."""
+        return int(self._L.nhp_debug_cycle_graph_kernels(self._h))
 
     def debug_set_plan_eager(self, n_waypoints):
         """Waypoints that come back with the status words (test aid: a small number exercises the second copy)."""

@@ -398,6 +398,11 @@ int nhp_render_obstacles_dt(nhp_planner *p, const uint8_t *hard, int on_device, 
     return NHP_OK;
 }
 
+int nhp_debug_cycle_graph_kernels(const nhp_planner *p)
+{
+    return (p && p->cycle_exec) ? p->cycle_graph_kernels : 0;
+}
+
 int nhp_debug_set_plan_eager(nhp_planner *p, int n_waypoints)
 {
     if (!p) return NHP_E_ARG;

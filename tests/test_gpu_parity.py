@@ -131,6 +131,13 @@ def test_distance_transform_and_soft_image_on_the_device(mods):
                 assert (p.collision_numpy() == Cv).all() and (p.soft_numpy() == Sv).all(), sc.name
                 p.run_nturn(sc.start, 2)
                 assert (p.cost_volume_numpy() == o.run(Cv, Sv, sc.start, 2)).all(), sc.name
+            if sc.n > 128 and k == 4.0:
+                # two cycles swept from the device-made soft image at full size (config 4)
+                o, fp = oracle_for(oracle, sc)
+                Cv, Sv = o.render(fp, sc.hard, soft, method="runs")
+                assert (p.collision_numpy() == Cv).all() and (p.soft_numpy() == Sv).all(), sc.name
+                p.run_nturn(sc.start, 2)
+                assert (p.cost_volume_numpy() == o.run(Cv, Sv, sc.start, 2)).all(), sc.name
             p.close()
             if sc.n > 128:
                 break
@@ -559,6 +566,48 @@ def test_first_cycle_with_the_sparse_launches(mods):
         p.close()
 
 
+@pytest.mark.slow
+def test_sparse_first_cycle_at_512_as_production_runs_it(mods):
+    """At 512^3 no CUDA graph is in use, so the one-tile first LF and the one-band-per-slice first SF are what every plan runs
+    (no profiling needed).  Starts are chosen so that the branches of those launches are all taken: a left-turn tile that wraps
+    the seam in x (tile column 0 and the last one) and one that does not, a start whose straight line lies in the last band of a
+    slice swept along x (I = 0) and of one swept along y (I = 1), a start on a diagonal heading, and random ones; hard (config 3)
+    and soft (config 4).  One cycle and two, whole volume."""
+    oracle, nhp = mods
+    for cfg, n_random in ((3, 2), (4, 1)):
+        sc = scenes.get_config(cfg)
+        o, fp = oracle_for(oracle, sc, threads=0)
+        Cv, Sv = o.render(fp, sc.hard, sc.soft, method="runs")
+        p = nhp.Planner.from_scene(sc)
+        assert p.cycle_graph_kernels() == 0
+        p.render_obstacles(sc.hard, sc.soft)
+        n, nt, mx, q = sc.n, sc.nt, sc.n - 1, sc.nt // 4
+        beta, B, I = o.beta.astype(np.int64), o.B.astype(np.int64), o.I
+        rng = np.random.default_rng(cfg)
+        flat = rng.integers(Cv.size, size=2000000)
+        flat = flat[Cv.reshape(-1)[flat] == 0]                           # free poses
+        tt, jj, ii = flat // (n * n), (flat // n) % n, flat % n
+        tile = ((ii - beta[tt]) & mx) >> 5                               # eq (18) inverted: tile column of the left-turn curve through the start
+        line = np.where(I[tt] == 0, (jj - B[tt, ii]) & mx, (ii - B[tt, jj]) & mx) >> 5      # eq (23) inverted: band of the straight line
+        wanted = [("tile column 0", tile == 0), ("last tile column", tile == n // 32 - 1), ("inner tile column", tile == n // 64),
+                  ("last band, I = 0", (line == n // 32 - 1) & (I[tt] == 0)), ("last band, I = 1", (line == n // 32 - 1) & (I[tt] == 1)),
+                  ("diagonal heading", tt % (nt // 8) == 0)] + [("random", np.ones(len(tt), bool))] * n_random
+        if cfg == 4:
+            wanted = wanted[::2]
+        for what, ok in wanted:
+            k = np.flatnonzero(ok)
+            assert len(k), what
+            k = k[rng.integers(len(k))]
+            start = (int(ii[k]), int(jj[k]), int(tt[k]))
+            for n_cycles in ((1, 2) if what in ("tile column 0", "last band, I = 1") else (1,)):
+                p.run_nturn(start, n_cycles)
+                p.status()
+                V = o.run(Cv, Sv, start, n_cycles)
+                got = p.cost_volume_numpy()
+                assert (got == V).all(), (sc.name, what, start, n_cycles, int((got != V).sum()))
+        p.close()
+
+
 def _full_config(mods, k, sample_render=20000):
     oracle, nhp = mods
     sc = scenes.get_config(k)
@@ -579,6 +628,12 @@ def _full_config(mods, k, sample_render=20000):
     if Sv is not None:
         assert (Sg == Sv).all()
     del Cg, Sg
+    if sc.n > 256:
+        # three whole Theta planes by the plain per-pose loop as well: an axis heading, a diagonal, a generic angle
+        for t in (0, sc.nt // 8, (5 * sc.nt) // 13 | 1)[(1 if sc.n > 512 else 0):]:      # config 5: seconds per plane, two planes
+            Cp, Sp = o.render_plane(fp, sc.hard, sc.soft, t)
+            assert (Cp == Cv[t]).all(), t
+            assert Sv is None or (Sp == Sv[t]).all(), t
     p.run_nturn(sc.start, sc.n_cycles)
     p.status()
     got = p.cost_volume_numpy()
