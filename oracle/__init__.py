@@ -71,6 +71,8 @@ def _load():
                                       C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_render_brute.argtypes = [C.c_void_p, C.POINTER(_Footprint)] + [C.c_void_p] * 4
         L.orc_render_brute_plane.argtypes = [C.c_void_p, C.POINTER(_Footprint), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_apply_lane.argtypes = [C.c_void_p] * 4
+        L.orc_apply_lane.restype = None
         L.orc_render_runs.argtypes = [C.c_void_p, C.POINTER(_Footprint)] + [C.c_void_p] * 4
         L.orc_footprint_offsets.argtypes = [C.c_void_p, C.POINTER(_Footprint), C.c_int, C.c_void_p, C.c_void_p, C.c_int]
         L.orc_sweep.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -210,6 +212,14 @@ class Oracle:
         if rc:
             raise OracleError(rc, "render_plane")
         return Cp, Sp
+
+    def apply_lane(self, Sv, lane_dir, lane_pen):
+        """Area / orientation penalty of DESIGN R28 folded into the soft volume Sv (uint8 [Theta][j][i]) in place; returns Sv."""
+        assert Sv.dtype == np.uint8 and Sv.flags.c_contiguous and Sv.shape == self.shape
+        lane_dir, lane_pen = np.ascontiguousarray(lane_dir, np.uint8), np.ascontiguousarray(lane_pen, np.uint8)
+        assert lane_dir.shape == (self.n, self.n) and lane_pen.shape == (self.n, self.n)
+        _load().orc_apply_lane(self._h, _ptr(Sv), _ptr(lane_dir), _ptr(lane_pen))
+        return Sv
 
     def footprint_offsets(self, fp: Footprint, t):
         cap = (2 * fp.radius() + 1) ** 2

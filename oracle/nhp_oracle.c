@@ -23,6 +23,10 @@
  *   graph sizes ... k_V / k_E of Table 1 (l.427) counted on the Dijkstra itself (tests/test_oracle_tables.py)
  *   render ........ brute force vs exact box dilation at axis angles; run renderer vs brute force
  *   back-track .... plan is a valid chain of curve segments whose cost sums to the reported cost
+ *   lane penalty .. (DESIGN R28, our definition) factor 16 = identity bit for bit, aligned heading unpenalised, opposite heading
+ *                   exactly x pen/16, symmetric and monotone in the angle and in pen, saturation; in free space a straight drive
+ *                   with the lane costs what it costs without the penalty and against it exactly pen/16 times that
+ *                   (tests/test_oracle_lane.py)
  *   orc_render_*'s footprint rasterisation rule (DESIGN R15) is OUR definition: "parity
  *   unpinned" against the paper, which gives no rule.
  *
@@ -330,6 +334,36 @@ int orc_render_brute_plane(const orc_ctx *c, const orc_footprint *fp, const uint
             if (S_out) S_out[(size_t)j * n + i] = soft ? ss : 16;
         }
     return 0;
+}
+
+/* Area / orientation penalty on the obstacle volume ("direction and area-based velocity penalties"; "the
+ * rendering ... handles any additional area and orientation related penalties", section VI l.338; Figure 19 l.463: "penalties
+ * to inform the planner not to use the reverse direction lane").  The paper gives no formula: reading DESIGN R28.
+ *   lane_dir[b][a]  preferred heading of pixel (a, b) in 1/256 turns (0 = +x, 64 = +y)
+ *   lane_pen[b][a]  Q4.4 factor (16 = 1.0; values below 16 count as 16) on the reciprocal velocity of a vehicle that faces the
+ *                   opposite way; in between the factor grows linearly with the angle
+ * For the pose (i, j, Theta), evaluated at its own pixel (the rear-axle cell):
+ *   h     = floor(256 Theta / N_theta)                      heading in 1/256 turns
+ *   delta = min((h - dir) mod 256, (dir - h) mod 256)       0 .. 128
+ *   f     = 16 + (((pen - 16) * 2 delta + 128) >> 8)        Q4.4, 16 .. pen
+ *   S    <- min(255, (S * f + 8) >> 4)                      Q4.4 product, rounded half up
+ * S: the rendered soft volume (R16), updated in place. */
+void orc_apply_lane(const orc_ctx *c, uint8_t *S, const uint8_t *lane_dir, const uint8_t *lane_pen)
+{
+    int n = c->n, nt = c->nt;
+    for (int t = 0; t < nt; t++) {
+        int h = (int)(((int64_t)256 * t) / nt);
+        for (int j = 0; j < n; j++)
+            for (int i = 0; i < n; i++) {
+                size_t px = (size_t)j * n + i, idx = ((size_t)t * n + j) * n + i;
+                int pen = lane_pen[px] < 16 ? 16 : lane_pen[px];
+                int d = (h - (int)lane_dir[px]) & 255;
+                int delta = d < 256 - d ? d : 256 - d;
+                int f = 16 + (((pen - 16) * 2 * delta + 128) >> 8);
+                int s = ((int)S[idx] * f + 8) >> 4;
+                S[idx] = (uint8_t)(s > 255 ? 255 : s);
+            }
+    }
 }
 
 /* Number of covered offsets for Theta (area check) and optional list output. */
