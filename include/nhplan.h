@@ -179,6 +179,22 @@ int nhp_set_box(nhp_planner *p, int f, int r, int s);
  * footprint, 16, 255) (DESIGN R16).  Errors: NHP_E_ARG, NHP_E_STATE (no footprint yet), NHP_E_CUDA. */
 int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *soft, int on_device);
 
+/* Area / orientation penalty ("direction and area-based velocity penalties"; "the rendering ... handles any
+ * additional area and orientation related penalties", section VI l.338; Figure 19 l.463: "penalties to inform the planner not
+ * to use the reverse direction lane and stay to the right").  The paper gives no formula; reading DESIGN R28:
+ *   lane_dir  N x N uint8, row = y, column = x: preferred heading of the pixel in 1/256 turns (0 = +x, 64 = +y, 128 = -x)
+ *   lane_pen  N x N uint8, Q4.4 factor (16 = 1.0 = no penalty; smaller values count as 16) on the reciprocal velocity of a
+ *             vehicle that faces the opposite way; in between the factor grows linearly with the angle
+ *   on_device 0: both are HOST memory, copied on the stream (keep them alive until the stream has passed the copy); 1: DEVICE
+ * The next nhp_render_obstacles / nhp_render_obstacles_dt folds it into the soft volume: for the pose (i, j, Theta), read at the
+ * pose's own pixel (i, j), h = floor(256 Theta / N_theta), delta = circular distance of h and lane_dir (0..128),
+ *   f = 16 + (((lane_pen - 16) * 2 delta + 128) >> 8),      S <- min(255, (S * f + 8) >> 4)
+ * with S the footprint maximum of the soft image (DESIGN R16).  It is a penalty on the vehicle's orientation (one obstacle
+ * volume over position and orientation, l.338): reversing along a lane while facing the right way is priced by dir_mult, not
+ * here.  Both pointers NULL: no penalty from the next render on.  Requires NHP_FLAG_SOFT (pass an all-16 soft image if there
+ * are no soft obstacle costs).  Errors: NHP_E_ARG, NHP_E_CUDA. */
+int nhp_set_lane_penalty(nhp_planner *p, const uint8_t *lane_dir, const uint8_t *lane_pen, int on_device);
+
 /* Steps 1-4 of PAPER.md:388-391 with the distance transform on the DEVICE (the paper runs steps 1-2 on the CPU):
  * the soft image is synthesised from the hard image and then rendered exactly as by nhp_render_obstacles.
  * Reading DESIGN R17 of "some function of the distance" (section VII l.342): with H = hard | wall (row 0 and

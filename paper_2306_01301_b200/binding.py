@@ -22,7 +22,7 @@ EXPORTS = ("nhp_query_sizes", "nhp_planner_create", "nhp_planner_destroy", "nhp_
            "nhp_run_nturn", "nhp_run_nturn_from", "nhp_reach_run", "nhp_reach_levels", "nhp_reach_count_volume", "nhp_reach_extract_path", "nhp_run_more",
            "nhp_cost_volume", "nhp_extract_path", "nhp_extract_path_goalset", "nhp_status", "nhp_index_to_pose", "nhp_pose_to_index",
            "nhp_debug_tables", "nhp_debug_footprint", "nhp_launch_count", "nhp_set_profiling", "nhp_kernel_times", "nhp_prof_dropped", "nhp_microbench_alu", "nhp_microbench_read",
-           "nhp_soft_from_hard_noalloc", "nhp_noalloc_last_error", "nhp_debug_set_plan_eager", "nhp_debug_cycle_graph_kernels")
+           "nhp_soft_from_hard_noalloc", "nhp_noalloc_last_error", "nhp_debug_set_plan_eager", "nhp_debug_cycle_graph_kernels", "nhp_set_lane_penalty")
 KERNEL_SLOTS = 17
 KERNEL_SLOT_NAMES = ("LF", "SF", "RB", "RF", "SB", "LB", "render_collision", "render_soft", "init_export",
                      "backtrack", "raster_pack", "turn_pair", "distance_transform", "reach_level", "straight_xrows", "straight_rows", "straight_sect")
@@ -81,6 +81,7 @@ def load_library():
         L.nhp_render_obstacles.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.nhp_render_obstacles_dt.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_double, C.c_void_p]
         L.nhp_debug_soft_image.argtypes = [C.c_void_p, C.c_void_p]
+        L.nhp_set_lane_penalty.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.nhp_debug_set_plan_eager.argtypes = [C.c_void_p, C.c_int]
         L.nhp_debug_cycle_graph_kernels.argtypes = [C.c_void_p]
         L.nhp_run_nturn.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int]
@@ -249,6 +250,24 @@ class Planner:
         assert soft is None or hd == sd
         self._keep = (hard, soft)                       # host buffers must outlive the async copy
         self._check(self._L.nhp_render_obstacles(self._h, hp, sp, hd), "render_obstacles")
+
+    def set_lane_penalty(self, lane_dir=None, lane_pen=None):
+        """Lane map of nhp_set_lane_penalty (area / orientation penalty, DESIGN R28): two (N, N) uint8 images, numpy (host path)
+        or CUDA tensors; None, None switches it off.  Takes effect at the next render_obstacles / render_obstacles_dt."""
+        if lane_dir is None and lane_pen is None:
+            self._check(self._L.nhp_set_lane_penalty(self._h, None, None, 0), "set_lane_penalty")
+            return
+        ptrs, dev = [], []
+        for a in (lane_dir, lane_pen):
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.uint8 and a.flags.c_contiguous and a.shape == (self.n, self.n)
+                ptrs.append(a.ctypes.data); dev.append(0)
+            else:
+                assert a.dtype == self.torch.uint8 and a.is_contiguous() and tuple(a.shape) == (self.n, self.n)
+                ptrs.append(a.data_ptr()); dev.append(int(a.is_cuda))
+        assert dev[0] == dev[1]
+        self._keep_lane = (lane_dir, lane_pen)             # host buffers must outlive the async copy
+        self._check(self._L.nhp_set_lane_penalty(self._h, ptrs[0], ptrs[1], dev[0]), "set_lane_penalty")
 
     def render_obstacles_dt(self, hard, k=4.0, dist_out=None):
         """Distance transform + soft image on the device, then rendering (nhp_render_obstacles_dt).

@@ -289,6 +289,7 @@ int nhp_planner_create(nhp_planner **out, int log2_n, int log2_ntheta, double R_
     alloc((void **)&p->d_hard, npx);
     alloc((void **)&p->d_soft, npx);
     if (w->flags & NHP_FLAG_SOFT) alloc((void **)&p->d_dtg, sizeof(int32_t) * npx);
+    if (w->flags & NHP_FLAG_SOFT) { alloc((void **)&p->d_lane_dir, npx); alloc((void **)&p->d_lane_pen, npx); }
     alloc((void **)&p->d_status, 2 * sp_bytes);
     alloc((void **)&p->d_goals, sizeof(int32_t) * 3 * NHP_MAX_GOALS);
     if (rc == NHP_OK && cudaMallocHost((void **)&p->h_status, sp_bytes) != cudaSuccess) rc = NHP_E_CUDA;
@@ -316,6 +317,7 @@ int nhp_planner_destroy(nhp_planner *p)
         if (p->cycle_graph) cudaGraphDestroy(p->cycle_graph);
         cudaFree(p->d_beta); cudaFree(p->d_B); cudaFree(p->d_lenq); cudaFree(p->d_IJ); cudaFree(p->d_rot); cudaFree(p->d_tlist); cudaFree(p->d_xl_tab);
         cudaFree(p->d_hard); cudaFree(p->d_soft); cudaFree(p->d_status); cudaFree(p->d_dtg); cudaFree(p->d_goals);
+        cudaFree(p->d_lane_dir); cudaFree(p->d_lane_pen);
         if (p->h_status) cudaFreeHost(p->h_status);
         for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     }
@@ -376,6 +378,21 @@ int nhp_render_obstacles(nhp_planner *p, const uint8_t *hard, const uint8_t *sof
     p->have_render = true;
     p->have_run = false;                  // both planners' results belong to the previous collision volume
     p->r_n_levels = -1;
+    return NHP_OK;
+}
+
+int nhp_set_lane_penalty(nhp_planner *p, const uint8_t *lane_dir, const uint8_t *lane_pen, int on_device)
+{
+    if (!p) return NHP_E_ARG;
+    if (!p->S || !p->d_lane_dir) return fail(p, NHP_E_ARG, "the planner has no soft volume (NHP_FLAG_SOFT)");
+    if (!lane_dir != !lane_pen) return fail(p, NHP_E_ARG, "lane_dir and lane_pen must both be given or both be NULL");
+    if (!lane_dir) { p->have_lane = false; return NHP_OK; }
+    DeviceGuard guard(p);
+    const size_t npx = (size_t)p->n * p->n;
+    const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(p->d_lane_dir, lane_dir, npx, kind, p->stream));
+    CU(cudaMemcpyAsync(p->d_lane_pen, lane_pen, npx, kind, p->stream));
+    p->have_lane = true;
     return NHP_OK;
 }
 

@@ -104,6 +104,8 @@ struct nhp_planner {
     bool have_footprint = false;
     // images
     uint8_t *d_hard = nullptr, *d_soft = nullptr;
+    uint8_t *d_lane_dir = nullptr, *d_lane_pen = nullptr;   // [n][n] lane map of nhp_set_lane_penalty (DESIGN R28), soft planners only
+    bool have_lane = false;
     int32_t *d_dtg = nullptr;      // [n][n] column distances of the distance transform (distance.cu), soft planners only
     // run decomposition of E_Theta and the sparse tables of the image rows (render.cu)
     int4 *d_runs = nullptr;        // (db, da_lo, second look-up offset, level) of every run, grouped by Theta

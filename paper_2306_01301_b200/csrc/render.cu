@@ -219,10 +219,30 @@ __device__ __forceinline__ uint4 soft_window(const uint4 *__restrict__ row, int 
     }
 }
 
+// Area / orientation penalty ("any additional area and orientation related penalties", Figure 19 l.463;
+// reading DESIGN R28) on four rendered soft values packed in a word: dir = preferred heading of the pose's own pixel in 1/256
+// turns, pen = Q4.4 factor paid in full when facing the opposite way, h = heading of the plane in 1/256 turns.
+//   delta = circular distance of h and dir (0 .. 128),  f = 16 + (((pen - 16) * 2 delta + 128) >> 8),  S <- min(255, (S f + 8) >> 4)
+__device__ __forceinline__ uint32_t lane_penalty4(uint32_t s4, uint32_t dir4, uint32_t pen4, int h)
+{
+    uint32_t out = 0;
+#pragma unroll
+    for (int b = 0; b < 4; b++) {
+        const int s = (s4 >> (8 * b)) & 255, dir = (dir4 >> (8 * b)) & 255, pen = max(16, (int)((pen4 >> (8 * b)) & 255));
+        const int d = (h - dir) & 255, delta = min(d, 256 - d);
+        const int f = 16 + (((pen - 16) * 2 * delta + 128) >> 8);
+        out |= (uint32_t)min(255, (s * f + 8) >> 4) << (8 * b);
+    }
+    return out;
+}
+
 // Sixteen poses per thread: per run two look-ups of 16 bytes each (four aligned 16-byte loads) instead of sixteen 4-byte
-// loads, and a quarter of the per-run bookkeeping per pose.
+// loads, and a quarter of the per-run bookkeeping per pose.  LANE: the penalty of R28 is applied to the sixteen values before
+// the one store (lane_dir / lane_pen: the N x N lane map, sixteen pixels per uint4).
+template <bool LANE>
 __global__ void __launch_bounds__(256) render_soft_kernel(uint4 *__restrict__ S16, const uint4 *__restrict__ Mk,
-                                                         const int4 *__restrict__ runs, const int32_t *__restrict__ run_off, int n)
+                                                         const int4 *__restrict__ runs, const int32_t *__restrict__ run_off, int n,
+                                                         const uint4 *__restrict__ lane_dir, const uint4 *__restrict__ lane_pen, int log2_nt)
 {
     extern __shared__ int4 srun[];
     const int nQ = n >> 4, mx = n - 1, mQ = nQ - 1;
@@ -243,8 +263,14 @@ __global__ void __launch_bounds__(256) render_soft_kernel(uint4 *__restrict__ S1
         const uint4 x = soft_window(row, a, mQ), y = soft_window(row, a + r.z, mQ);
         max16_add(acc, 0, x.x, y.x); max16_add(acc, 1, x.y, y.y); max16_add(acc, 2, x.z, y.z); max16_add(acc, 3, x.w, y.w);
     }
-    S16[((size_t)t * n + j) * nQ + iQ] = make_uint4(acc.e[0] | (acc.o[0] << 8), acc.e[1] | (acc.o[1] << 8), acc.e[2] | (acc.o[2] << 8),
-                                                    acc.e[3] | (acc.o[3] << 8));
+    uint4 s = make_uint4(acc.e[0] | (acc.o[0] << 8), acc.e[1] | (acc.o[1] << 8), acc.e[2] | (acc.o[2] << 8), acc.e[3] | (acc.o[3] << 8));
+    if (LANE) {
+        const uint4 d = lane_dir[(size_t)j * nQ + iQ], q = lane_pen[(size_t)j * nQ + iQ];
+        const int h = (t << 8) >> log2_nt;                       // floor(256 Theta / N_theta)
+        s = make_uint4(lane_penalty4(s.x, d.x, q.x, h), lane_penalty4(s.y, d.y, q.y, h), lane_penalty4(s.z, d.z, q.z, h),
+                       lane_penalty4(s.w, d.w, q.w, h));
+    }
+    S16[((size_t)t * n + j) * nQ + iQ] = s;
 }
 
 int launch_render(nhp_planner *p, bool soft)
@@ -272,8 +298,11 @@ int launch_render(nhp_planner *p, bool soft)
         ProfScope prof(p, 7);
         const int nQ = n / 16;
         const dim3 block(nQ < 32 ? nQ : 32, 8);
-        render_soft_kernel<<<dim3(nQ / block.x, n / 8, p->nt), block, smem, p->stream>>>((uint4 *)p->S, (const uint4 *)p->d_Mk,
-                                                                                       p->d_runs, p->d_run_off, n);
+        const dim3 grid(nQ / block.x, n / 8, p->nt);
+        if (p->have_lane) render_soft_kernel<true><<<grid, block, smem, p->stream>>>((uint4 *)p->S, (const uint4 *)p->d_Mk, p->d_runs, p->d_run_off, n,
+                                                                                   (const uint4 *)p->d_lane_dir, (const uint4 *)p->d_lane_pen, p->log2_nt);
+        else render_soft_kernel<false><<<grid, block, smem, p->stream>>>((uint4 *)p->S, (const uint4 *)p->d_Mk, p->d_runs, p->d_run_off, n,
+                                                                       nullptr, nullptr, p->log2_nt);
         launches++;
         launches += launch_soft_layouts(p);
     }

@@ -272,3 +272,57 @@ def random_scene(log2_n, log2_nt, R, seed, n_rects=6, max_side=None, vehicle=(4,
     return Scene(f"rand_{log2_n}_{log2_nt}_{seed}", log2_n, log2_nt, float(R), n_cycles,
                  tuple(ct) if ct is not None else counting_weights(R), tuple(dm), hard,
                  soft_from_hard(hard) if soft else None, mask, ou, ov, start, goal, flags=flags)
+
+
+def random_lane_map(n: int, seed: int, max_pen: int = 80):
+    """Lane map for parity tests (DESIGN R28): piecewise-constant 8 x 8 blocks of random preferred headings and Q4.4 factors
+    (a quarter of the blocks carry no penalty, a few carry factors below 16, which count as 16)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    b = max(1, n // 8)
+    d = np.kron(rng.integers(0, 256, size=(8, 8)), np.ones((b, b), np.int64)).astype(np.uint8)
+    pen = rng.integers(8, max_pen + 1, size=(8, 8))
+    pen[rng.random((8, 8)) < 0.25] = 16
+    return np.ascontiguousarray(d[:n, :n]), np.ascontiguousarray(np.kron(pen, np.ones((b, b), np.int64)).astype(np.uint8)[:n, :n])
+
+
+def two_lane_road(log2_n: int = 9, log2_nt: int = 9, seed: int = 6):
+    """A scene shaped like Figure 19 ('penalties to inform the planner not to use the reverse direction lane
+    and stay to the right'): a horizontal two-lane road across the grid between two walls with a few parked boxes along its
+    edges; the lower lane (smaller y) runs towards +x, the upper lane towards -x, driving a lane the wrong way costs a factor 4,
+    and a strip along the centre line costs 1.5 whichever way one faces (an area penalty: lane_pen 24 with the heading of the
+    lane it lies in).  Vehicle 20 x 9, R = 40 at 512 (scaled with N), N_T = 6, reverse x2; start in the lower lane at the left
+    facing +x, goal in the upper lane at the left facing -x (a U-turn further down the road), extra goals along both lanes.
+    -> (Scene, lane_dir, lane_pen)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n, nt = 1 << log2_n, 1 << log2_nt
+    s = n / 512.0
+    L, W, R = max(4, int(round(20 * s))), max(2, int(round(9 * s))), max(4.0, 40.0 * s)
+    half = int(round(70 * s))                                   # half width of the road
+    mid = n // 2
+    hard = np.zeros((n, n), np.uint8)
+    hard[: mid - half, :] = 1
+    hard[mid + half:, :] = 1
+    for _ in range(6):                                          # parked boxes along the kerbs
+        x0 = int(rng.integers(int(40 * s), n - int(60 * s)))
+        if rng.random() < 0.5:
+            _fill_rect(hard, x0, mid - half, L + 2, W + 1)
+        else:
+            _fill_rect(hard, x0, mid + half - W - 1, L + 2, W + 1)
+    lane_dir = np.zeros((n, n), np.uint8)
+    lane_dir[mid:, :] = 128                                     # upper lane: heading -x
+    lane_pen = np.full((n, n), 64, np.uint8)                    # x4 against the lane
+    strip = max(1, int(round(4 * s)))
+    lane_pen[mid - strip: mid + strip, :] = 24
+    lane_dir[mid - strip: mid, :] = 128                         # the centre strip is charged to whoever drives ALONG it: its
+    lane_dir[mid: mid + strip, :] = 0                           # 'preferred' heading is the opposite lane's
+    mask, ou, ov = box_mask(L, W)
+    soft = soft_from_hard(hard)
+    y_lo, y_hi = mid - half // 2, mid + half // 2
+    start = (int(60 * s), y_lo, 0)
+    goal = (int(60 * s), y_hi, nt // 2)
+    extra = [(int(x), y_lo, 0) for x in np.linspace(100 * s, n - 60 * s, 6)] + [(int(x), y_hi, nt // 2) for x in np.linspace(100 * s, n - 60 * s, 6)]
+    dm = [256] * 6
+    dm[LB] = dm[SB] = dm[RB] = 512
+    sc = Scene(f"two_lane_road_{n}", log2_n, log2_nt, float(R), 6, counting_weights(R / 4), tuple(dm), hard, soft, mask, ou, ov,
+               start, goal, extra_goals=extra)
+    return sc, lane_dir, lane_pen

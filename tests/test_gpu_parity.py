@@ -566,6 +566,88 @@ def test_first_cycle_with_the_sparse_launches(mods):
         p.close()
 
 
+def test_lane_penalty_small_scenes(mods):
+    """nhp_set_lane_penalty (area / orientation penalty, DESIGN R28): the soft volume with the penalty
+    folded in, the sweeps over it and the plans are the oracle's, bit for bit; host and device lane maps; through both render
+    calls; switching it off restores the plain volume; N_theta below, at and above 256 (the heading is taken in 1/256 turns)."""
+    oracle, nhp = mods
+    import torch
+    cases = [scenes.random_scene(5, 5, 4, 61, soft=True, reverse_mult=512), scenes.random_scene(6, 6, 8, 62, vehicle=(6, 3), soft=True),
+             scenes.random_scene(7, 8, 9, 63, vehicle=(9, 4), n_rects=20, soft=True, n_cycles=2),
+             scenes.random_scene(5, 10, 6, 64, soft=True, n_cycles=2)]
+    for k, sc in enumerate(cases):
+        lane_dir, lane_pen = scenes.random_lane_map(sc.n, 100 + k)
+        o, fp = oracle_for(oracle, sc)
+        Cv, S0 = o.render(fp, sc.hard, sc.soft, method="brute")
+        S1 = o.apply_lane(S0.copy(), lane_dir, lane_pen)
+        assert (S1 != S0).any()
+        p = nhp.Planner.from_scene(sc)
+        if k % 2:
+            p.set_lane_penalty(torch.from_numpy(lane_dir).to(p.device), torch.from_numpy(lane_pen).to(p.device))
+        else:
+            p.set_lane_penalty(lane_dir, lane_pen)
+        p.render_obstacles(sc.hard, sc.soft)
+        assert (p.collision_numpy() == Cv).all() and (p.soft_numpy() == S1).all(), sc.name
+        p.run_nturn(sc.start, sc.n_cycles)
+        V = o.run(Cv, S1, sc.start, sc.n_cycles)
+        assert (p.cost_volume_numpy() == V).all(), sc.name
+        tj, jj, ij = np.nonzero(V != INF)
+        rng = np.random.default_rng(k)
+        for g in rng.integers(len(tj), size=10):
+            goal = (int(ij[g]), int(jj[g]), int(tj[g]))
+            assert p.extract_path(goal) == o.backtrack(V, Cv, S1, sc.start, goal), (sc.name, goal)
+        # the device distance transform path renders with the same epilogue
+        _, _, soft_dt = oracle.soft_from_hard(sc.hard, 4.0)
+        _, Sdt = o.render(fp, sc.hard, soft_dt, method="brute")
+        p.render_obstacles_dt(sc.hard, 4.0)
+        assert (p.soft_numpy() == o.apply_lane(Sdt.copy(), lane_dir, lane_pen)).all(), sc.name
+        # off again
+        p.set_lane_penalty(None, None)
+        p.render_obstacles(sc.hard, sc.soft)
+        assert (p.soft_numpy() == S0).all(), sc.name
+        with pytest.raises(nhp.NhpError) as e:
+            p._check(p._L.nhp_set_lane_penalty(p._h, lane_dir.ctypes.data, None, 0), "set_lane_penalty")
+        assert e.value.code == -1
+        p.close()
+    sc = scenes.random_scene(5, 5, 4, 1)                      # no soft volume: refused
+    p = nhp.Planner.from_scene(sc)
+    with pytest.raises(nhp.NhpError) as e:
+        p.set_lane_penalty(*scenes.random_lane_map(sc.n, 1))
+    assert e.value.code == -1
+    p.close()
+
+
+@pytest.mark.slow
+def test_lane_penalty_two_lane_road_512(mods):
+    """A 512^3 scene shaped like Figure 19: two lanes, wrong-way factor 4, centre strip 1.5.  Soft volume, cost
+    volume and plans against the oracle; and what the penalty is for: goals down the start's own lane cost what they cost
+    without it, the goal in the opposite lane (a U-turn) costs more."""
+    oracle, nhp = mods
+    sc, lane_dir, lane_pen = scenes.two_lane_road(9, 9)
+    o, fp = oracle_for(oracle, sc, threads=0)
+    Cv, S0 = o.render(fp, sc.hard, sc.soft, method="runs")
+    S1 = o.apply_lane(S0.copy(), lane_dir, lane_pen)
+    p = nhp.Planner.from_scene(sc)
+    p.render_obstacles(sc.hard, sc.soft)
+    p.run_nturn(sc.start, sc.n_cycles)
+    V0 = p.cost_volume_numpy().copy()
+    p.set_lane_penalty(lane_dir, lane_pen)
+    p.render_obstacles(sc.hard, sc.soft)
+    assert (p.collision_numpy() == Cv).all() and (p.soft_numpy() == S1).all()
+    p.run_nturn(sc.start, sc.n_cycles)
+    p.status()
+    V = o.run(Cv, S1, sc.start, sc.n_cycles)
+    got = p.cost_volume_numpy()
+    assert (got == V).all(), int((got != V).sum())
+    for goal in [sc.goal] + sc.extra_goals:
+        assert p.extract_path(goal) == o.backtrack(V, Cv, S1, sc.start, goal), goal
+    same_lane = [g for g in sc.extra_goals if g[2] == 0][:-1]          # the last one sits next to the end wall (soft costs differ there)
+    assert all(V[g[2], g[1], g[0]] == V0[g[2], g[1], g[0]] for g in same_lane)
+    g = sc.goal
+    assert V[g[2], g[1], g[0]] > V0[g[2], g[1], g[0]]
+    p.close()
+
+
 @pytest.mark.slow
 def test_sparse_first_cycle_at_512_as_production_runs_it(mods):
     """At 512^3 no CUDA graph is in use, so the one-tile first LF and the one-band-per-slice first SF are what every plan runs
