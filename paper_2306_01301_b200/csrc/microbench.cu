@@ -3,6 +3,7 @@
 // (nhp_arrive / nhp_keep / nhp_gate); this kernel issues nothing else, in `CH` independent dependency chains per
 // thread, 8 warps per SM sub-partition, and is timed with CUDA events on the handle's stream.
 #include "nhp_internal.cuh"
+#include "../../include/nhplan_probe.h"
 
 // The probes' own sink word (device code names it directly): written only if an impossible value turns up, which keeps the
 // measured instructions alive without touching anything of the planner's.

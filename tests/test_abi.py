@@ -15,7 +15,7 @@ def lib():
 
 
 def declared_symbols():
-    src = open(os.path.join(ROOT, "include", "nhplan.h")).read()
+    src = "".join(open(os.path.join(ROOT, "include", f)).read() for f in sorted(os.listdir(os.path.join(ROOT, "include"))) if f.endswith(".h"))
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(nhp_[a-z_0-9]+)\s*\(", src)))
 
